@@ -1,0 +1,374 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+The paper (arxiv 1004.1302) prints no worked numerical example and no pixel value, so the pins
+are closed forms, invariants, special cases and brute force:
+  * true 3-D ray integration of the Gaussian density of PAPER.md:69 (P1, camera conventions)
+  * closed-form flux of a truncated Gaussian splat and energy conservation (P2, P3)
+  * permutation and scale invariance (P4, P10)
+  * RK4 integration of the transfer equation, Eq. (1) (P5, P6)
+  * absorb == additive when A == E; front-to-back == back-to-front (P7, P8)
+  * image orientation, culling, look-up table nodes, tie order (P9, P11, P12)
+None of these reuses an oracle routine to produce its expected value.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import ABSORB, ADDITIVE
+
+from helpers import cam, const_lut, mk
+
+SQRT_PI = np.sqrt(np.pi)
+
+
+def _basis(c):
+    """Right-handed pinhole basis of DESIGN.md R1/R2, restated independently of the oracle."""
+    eye, look, up = (np.array(v, np.float32).astype(np.float64) for v in (c.eye, c.lookat, c.up))
+    fwd = look - eye
+    fwd /= np.linalg.norm(fwd)
+    right = np.cross(fwd, up)
+    right /= np.linalg.norm(right)
+    upv = np.cross(right, fwd)
+    F = 0.5 * c.width / np.tan(np.deg2rad(float(np.float32(c.fov_deg))) / 2)
+    return eye, right, upv, fwd, F
+
+
+# ------------------------------------------------------------------------------------------------
+# P1 + conventions: the image of ONE particle equals the numerically integrated column density of
+# rho = I exp(-|x - p|^2 / r^2) along the true 3-D ray through each pixel centre.
+# A narrow field of view makes the paraxial reading R3 exact to ~2e-4.
+# ------------------------------------------------------------------------------------------------
+def test_p1_true_ray_integration_single_particle():
+    c = cam(eye=(0, 0, -200.0), fov=0.5, w=33, h=33)
+    w = mk([(0.10, -0.05, 0.30, 0.12, 0.7, 0.0)], c, lut_e=const_lut((1.0, 0.5, 0.25)), support_f=3.0)
+    img = oracle.render(w, raw=True)
+    eye, right, upv, fwd, F = _basis(c)
+    p = np.array([w.x[0], w.y[0], w.z[0]], np.float64)
+    r, I = float(w.r[0]), float(w.I[0])
+    tab, ok = oracle.splat_table(w)
+    assert ok[0] == 1
+    sxo, syo, sgo, Ro = tab[0, :4]
+    n_cov = 0
+    for j in range(c.height):
+        for i in range(c.width):
+            d = fwd * F + right * (i + 0.5 - c.width / 2) + upv * (c.height / 2 - (j + 0.5))
+            d /= np.linalg.norm(d)
+            tc = np.dot(p - eye, d)
+            t = np.linspace(tc - 9 * r, tc + 9 * r, 4001)
+            pts = eye[None, :] + t[:, None] * d[None, :]
+            rho = I * np.exp(-np.sum((pts - p) ** 2, axis=1) / r ** 2)
+            tau = float(np.sum(rho[1:] + rho[:-1]) * 0.5 * (t[1] - t[0]))
+            b = np.linalg.norm((p - eye) - tc * d)           # true impact parameter
+            dd = np.hypot(i + 0.5 - sxo, j + 0.5 - syo)
+            if abs(dd - Ro) < 0.05:                          # rim pixels: either answer is legal here
+                continue
+            if b <= 3.0 * r:
+                n_cov += 1
+                np.testing.assert_allclose(img[j, i], tau * np.array([1.0, 0.5, 0.25]), rtol=5e-4, atol=0)
+            else:
+                assert np.all(img[j, i] == 0.0)
+    assert n_cov > 100
+
+
+# ------------------------------------------------------------------------------------------------
+# P2: flux of one splat fully inside the frame:
+#     sum_pixels S_c = a_c pi sigma_s^2 (1 - exp(-f^2)),  a_c = E_c I r sqrt(pi)
+# (integral of the truncated 2-D Gaussian; grid sampling error 2 exp(-pi^2 sigma_s^2) + rim term).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("f,tol", [(3.0, 3e-4), (5.0, 1e-9)])
+@pytest.mark.parametrize("off", [(0.0, 0.0), (0.013, -0.007), (0.0041, 0.0093)])
+def test_p2_flux_closed_form(f, tol, off):
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=96, h=96)
+    w = mk([(off[0], off[1], 0.0, 0.1, 0.8, 0.0)], c, lut_e=const_lut((0.9, 0.6, 0.3)), support_f=f)
+    S = oracle.render(w, raw=True)
+    F = 48.0 / np.tan(np.deg2rad(10.0))
+    sigma_s = F * float(w.r[0]) / 10.0
+    assert sigma_s > 2.0
+    a = np.array([0.9, 0.6, 0.3], np.float32).astype(np.float64) * float(w.I[0]) * float(w.r[0]) * SQRT_PI
+    expect = a * np.pi * sigma_s ** 2 * (1.0 - np.exp(-f * f))
+    np.testing.assert_allclose(S.sum(axis=(0, 1)), expect, rtol=tol)
+
+
+# P3: energy conservation for many splats inside the frame
+def test_p3_energy_conservation_many_splats():
+    rs = np.random.RandomState(7)
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=128, h=128)
+    F = 64.0 / np.tan(np.deg2rad(10.0))
+    n = 200
+    z = rs.uniform(-1.0, 1.0, n)
+    zc = z + 10.0
+    sig_s = rs.uniform(2.0, 6.0, n)
+    r = sig_s * zc / F
+    # keep the whole disc (f = 3) inside the frame
+    half = (64.0 - 3.0 * sig_s - 1.0) * zc / F
+    x = rs.uniform(-1, 1, n) * half
+    y = rs.uniform(-1, 1, n) * half
+    I = rs.uniform(0.5, 1.0, n)
+    cv = rs.uniform(0, 1, n)
+    lut = np.array([[0.2, 0.5, 0.9], [1.0, 0.3, 0.1]], np.float32)
+    w = mk(np.stack([x, y, z, r, I, cv], 1), c, lut_e=lut, brightness=(0.7,))
+    S = oracle.render(w, raw=True)
+    cvf = w.colval.astype(np.float64)
+    E = np.float64(np.float32(0.7)) * ((1 - cvf)[:, None] * lut[0].astype(np.float64) + cvf[:, None] * lut[1].astype(np.float64))
+    sig = F * w.r.astype(np.float64) / (w.z.astype(np.float64) + 10.0)
+    a = E * (w.I.astype(np.float64) * w.r.astype(np.float64) * SQRT_PI)[:, None]
+    expect = (a * (np.pi * sig ** 2 * (1 - np.exp(-9.0)))[:, None]).sum(axis=0)
+    np.testing.assert_allclose(S.sum(axis=(0, 1)), expect, rtol=3e-4)
+
+
+# P4: the additive image does not depend on the particle order
+def test_p4_permutation_invariance():
+    import workloads
+    w = workloads.make("C1", 5000, width=64, height=64)
+    S = oracle.render(w, raw=True)
+    perm = np.random.RandomState(3).permutation(w.n)
+    w2 = mk(np.stack([w.x[perm], w.y[perm], w.z[perm], w.r[perm], w.I[perm], w.colval[perm]], 1), w.camera,
+            lut_e=w.lut_e, brightness=w.brightness)
+    S2 = oracle.render(w2, raw=True)
+    np.testing.assert_allclose(S2, S, rtol=1e-12, atol=1e-300)
+    assert S.max() > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# brute force: RK4 integration of Eq. (1) along depth, for every pixel of a tiny image,
+# density of particle p along the ray = I_p exp(-d^2/sigma_s^2) exp(-(s - z_p)^2 / r_p^2) [d <= R]
+# ------------------------------------------------------------------------------------------------
+def _ode_image(w, c, E, A, n_steps=6000):
+    eye, right, upv, fwd, F = _basis(c)
+    P = np.stack([w.x, w.y, w.z], 1).astype(np.float64) - eye[None]
+    zc = P @ fwd
+    sx = c.width / 2 + F * (P @ right) / zc
+    sy = c.height / 2 - F * (P @ upv) / zc
+    sg = F * w.r.astype(np.float64) / zc
+    R = w.support_f * sg
+    rr = w.r.astype(np.float64)
+    jj, ii = np.meshgrid(np.arange(c.height) + 0.5, np.arange(c.width) + 0.5, indexing="ij")
+    d2 = (ii[None] - sx[:, None, None]) ** 2 + (jj[None] - sy[:, None, None]) ** 2
+    amp = w.I.astype(np.float64)[:, None, None] * np.exp(-d2 / sg[:, None, None] ** 2) * (d2 <= (R ** 2)[:, None, None])
+    s_far, s_near = (zc + 7 * rr).max(), (zc - 7 * rr).min()
+    h = (s_far - s_near) / n_steps            # step of the propagation coordinate (far -> near)
+
+    def rhs(s, Iv):                            # Iv: (H, W, 3)
+        out = np.zeros_like(Iv)
+        for p in range(len(zc)):
+            rho = amp[p] * np.exp(-((s - zc[p]) ** 2) / rr[p] ** 2)
+            out += (E[p][None, None, :] - A[p][None, None, :] * Iv) * rho[:, :, None]
+        return out
+
+    Iv = np.zeros((c.height, c.width, 3))
+    s = s_far
+    for _ in range(n_steps):
+        k1 = rhs(s, Iv)
+        k2 = rhs(s - h / 2, Iv + h * k1 / 2)
+        k3 = rhs(s - h / 2, Iv + h * k2 / 2)
+        k4 = rhs(s - h, Iv + h * k3)
+        Iv = Iv + h * (k1 + 2 * k2 + 2 * k3 + k4) / 6
+        s -= h
+    return Iv
+
+
+_LUT2E = np.array([[0.2, 0.5, 0.9], [1.0, 0.3, 0.1]], np.float32)
+_LUT2A = np.array([[1.5, 0.1, 0.6], [0.05, 0.9, 2.0]], np.float32)
+
+
+def _lerp(lut, cv):
+    cv = np.asarray(cv, np.float32).astype(np.float64)
+    return (1 - cv)[:, None] * lut[0].astype(np.float64) + cv[:, None] * lut[1].astype(np.float64)
+
+
+def test_p5_rk4_additive_overlapping():
+    c = cam(eye=(0, 0, -10.0), fov=6.0, w=8, h=8)
+    pts = [(0.00, 0.00, 0.00, 0.10, 2.0, 0.0), (0.05, -0.04, 0.05, 0.16, 1.2, 0.5),
+           (-0.08, 0.06, -0.08, 0.12, 3.0, 1.0), (0.10, 0.10, 0.02, 0.05, 4.0, 0.25),
+           (-0.12, -0.10, 0.20, 0.20, 0.9, 0.75)]
+    w = mk(pts, c, lut_e=_LUT2E, brightness=(1.3,))
+    E = np.float64(np.float32(1.3)) * _lerp(_LUT2E, w.colval)
+    ref = _ode_image(w, c, E, E)
+    out = oracle.render(w)                      # 1 - exp(-S)
+    assert out.max() > 0.2
+    np.testing.assert_allclose(out, ref, rtol=1e-7, atol=1e-9)
+
+
+def _disjoint_points():
+    # separated in depth by more than 6 (r_p + r_q) so that the slab reading R10 is exact
+    return [(0.00, 0.00, -3.0, 0.10, 2.0, 0.0), (0.05, -0.04, 0.0, 0.16, 1.2, 0.5),
+            (-0.08, 0.06, 3.0, 0.12, 3.0, 1.0), (0.02, 0.03, 6.0, 0.20, 1.5, 0.25)]
+
+
+def test_p6_rk4_absorb_disjoint_and_order_matters():
+    c = cam(eye=(0, 0, -12.0), fov=6.0, w=8, h=8)
+    w = mk(_disjoint_points(), c, lut_e=_LUT2E, lut_a=_LUT2A, brightness=(1.3,), abs_brightness=(0.8,), mode=ABSORB)
+    E = np.float64(np.float32(1.3)) * _lerp(_LUT2E, w.colval)
+    A = np.float64(np.float32(0.8)) * _lerp(_LUT2A, w.colval)
+    ref = _ode_image(w, c, E, A, n_steps=12000)
+    out = oracle.render(w)
+    assert out.max() > 0.2
+    np.testing.assert_allclose(out, ref, rtol=2e-7, atol=1e-9)
+    # reversing the depth order (mirror the particles through the lookat plane) changes the image
+    pts2 = [(x, y, 3.0 - z, r, I, cv) for (x, y, z, r, I, cv) in _disjoint_points()]
+    w2 = mk(pts2, c, lut_e=_LUT2E, lut_a=_LUT2A, brightness=(1.3,), abs_brightness=(0.8,), mode=ABSORB)
+    out2 = oracle.render(w2)
+    assert np.abs(out2 - out).max() > 1e-2
+
+
+def test_p7_absorb_with_a_equal_e_is_additive():
+    import workloads
+    w = workloads.make("C1", 3000, width=48, height=48)
+    w.brightness = [w.brightness[0] * 3.0]
+    add = oracle.render(w, mode=ADDITIVE)
+    w.lut_a = w.lut_e.copy()
+    w.abs_brightness = list(w.brightness)
+    ab = oracle.render(w, mode=ABSORB)
+    assert add.max() > 0.5
+    np.testing.assert_allclose(ab, add, rtol=1e-11, atol=1e-14)
+
+
+def test_p8_front_to_back_equals_back_to_front():
+    """The (C, T) recurrence nearest-first, written out here, equals the oracle's far-to-near form."""
+    import workloads
+    w = workloads.make("C4", 2000, width=32, height=32)
+    c = w.camera
+    out = oracle.render(w)
+    tab, ok = oracle.splat_table(w)
+    pr = oracle.project_f32(w)
+    vis = ok.astype(bool)
+    key = pr["zkey"].astype(np.int64).copy()
+    # particles the canonical box test dropped but the double table kept need a key too
+    order = [p for p in np.lexsort((np.arange(w.n), key)) if vis[p] and pr["visible"][p]]
+    missing = [p for p in range(w.n) if vis[p] and not pr["visible"][p]]
+    Cimg = np.zeros((c.height, c.width, 3))
+    Timg = np.ones((c.height, c.width, 3))
+    jj, ii = np.meshgrid(np.arange(c.height) + 0.5, np.arange(c.width) + 0.5, indexing="ij")
+    for p in order:
+        sx, sy, sg, R, tau0 = tab[p, :5]
+        d2 = (ii - sx) ** 2 + (jj - sy) ** 2
+        tau = np.where(d2 <= R * R, tau0 * np.exp(-d2 / sg ** 2), 0.0)[:, :, None]
+        u = tab[p, 8:11][None, None, :] * tau
+        phi = np.where(u > 0, -np.expm1(-u) / np.where(u > 0, u, 1.0), 1.0)
+        Cimg += Timg * tab[p, 5:8][None, None, :] * tau * phi
+        Timg *= np.exp(-u)
+    # the few splats outside the canonical box touch no pixel centre: they cannot change the image
+    for p in missing:
+        sx, sy, sg, R = tab[p, :4]
+        assert not np.any((ii - sx) ** 2 + (jj - sy) ** 2 <= R * R)
+    assert out.max() > 0.05
+    np.testing.assert_allclose(out, Cimg, rtol=1e-10, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------
+# P9: conventions R1, R2, R4, R5, R6
+# ------------------------------------------------------------------------------------------------
+def test_p9_orientation_and_culling():
+    c = cam(eye=(0, 0, -10.0), lookat=(0, 0, 0), up=(0, 1, 0), fov=20.0, w=65, h=65)
+    eye, right, upv, fwd, F = _basis(c)
+    base = dict(lut_e=const_lut((1, 1, 1)))
+
+    def centroid(pt):
+        S = oracle.render(mk([pt], c, **base), raw=True)[:, :, 0]
+        jj, ii = np.meshgrid(np.arange(65) + 0.5, np.arange(65) + 0.5, indexing="ij")
+        return (S * ii).sum() / S.sum(), (S * jj).sum() / S.sum(), S
+
+    cx, cy, S = centroid((0, 0, 0, 0.05, 1, 0))
+    assert abs(cx - 32.5) < 1e-9 and abs(cy - 32.5) < 1e-9      # optical axis -> (W/2, H/2)
+    ux, uy, _ = centroid(tuple(0.3 * upv) + (0.05, 1, 0))
+    assert uy < cy - 3 and abs(ux - cx) < 1e-6                    # +up -> smaller row index
+    rx, ry, _ = centroid(tuple(0.3 * right) + (0.05, 1, 0))
+    assert rx > cx + 3 and abs(ry - cy) < 1e-6                    # +right (= fwd x up) -> larger column
+    # expected displacement F * 0.3 / 10 pixels
+    assert abs((rx - cx) - F * 0.3 / 10.0) < 1e-3
+    # behind the camera, off-frame, inside the near plane, invalid fields: exactly zero
+    for pt in [(0, 0, -20.0, 0.05, 1, 0), (50.0, 0, 0, 0.05, 1, 0), (0, 0, -10.0 + 0.005, 0.05, 1, 0),
+               (0, 0, 0, -0.05, 1, 0), (0, 0, 0, 0.0, 1, 0), (np.nan, 0, 0, 0.05, 1, 0),
+               (0, 0, 0, 0.05, np.inf, 0), (0, 0, 0, 0.05, 1, np.nan)]:
+        assert np.all(oracle.render(mk([pt], c, **base), raw=True) == 0.0)
+    # a splat too small to reach a pixel centre contributes nothing (R4); on a pixel centre it
+    # lights exactly that pixel with its peak value a = E I r sqrt(pi)
+    tiny = 1e-4
+    Sz = oracle.render(mk([(0, 0, 0, tiny, 1, 0)], cam(eye=(0, 0, -10.0), fov=20.0, w=64, h=64), **base), raw=True)
+    assert np.all(Sz == 0.0)                                      # W even: the axis falls between pixels
+    So = oracle.render(mk([(0, 0, 0, tiny, 1, 0)], c, **base), raw=True)
+    assert np.count_nonzero(So[:, :, 0]) == 1
+    np.testing.assert_allclose(So[32, 32], np.float64(np.float32(tiny)) * SQRT_PI, rtol=1e-12)
+
+
+def test_p9_type_out_of_range_is_culled():
+    c = cam(w=16, h=16)
+    w = mk([(0, 0, 0, 0.2, 1, 0), (0, 0, 0, 0.2, 1, 0)], c, lut_e=const_lut((1, 1, 1), n_types=2),
+           brightness=(1.0, 2.0), types=[1, 3])
+    w1 = mk([(0, 0, 0, 0.2, 1, 0)], c, lut_e=const_lut((1, 1, 1), n_types=2), brightness=(1.0, 2.0), types=[1])
+    np.testing.assert_array_equal(oracle.render(w, raw=True), oracle.render(w1, raw=True))
+
+
+# P10: tau is proportional to I r, so scaling every length by s and I by 1/s leaves the image unchanged
+def test_p10_scale_invariance():
+    c = cam(eye=(0.5, 0.25, -8.0), lookat=(0.5, 0.25, 0.0), fov=16.0, w=40, h=40)
+    rs = np.random.RandomState(11)
+    pts = np.stack([rs.uniform(-0.5, 1.5, 40), rs.uniform(-0.5, 1.0, 40), rs.uniform(-1, 1, 40),
+                    rs.uniform(0.02, 0.2, 40), rs.uniform(0.5, 1, 40), rs.uniform(0, 1, 40)], 1)
+    w = mk(pts, c, lut_e=_LUT2E, lut_a=_LUT2A, mode=ABSORB, z_near=0.01)
+    s = 4.0                                                       # power of two: exact in fp32
+    pts2 = np.stack([w.x * s, w.y * s, w.z * s, w.r * s, w.I / s, w.colval], 1)
+    c2 = cam(eye=tuple(np.array(c.eye) * s), lookat=tuple(np.array(c.lookat) * s), fov=16.0, w=40, h=40)
+    w2 = mk(pts2, c2, lut_e=_LUT2E, lut_a=_LUT2A, mode=ABSORB, z_near=0.01 * s)
+    for mode in (ADDITIVE, ABSORB):
+        np.testing.assert_allclose(oracle.render(w2, mode=mode), oracle.render(w, mode=mode), rtol=1e-12, atol=1e-15)
+
+
+# P11: look-up table (R7)
+def test_p11_lut_nodes_midpoints_clamp():
+    c = cam(w=16, h=16)
+    lut = np.array([[0.1, 0.2, 0.3], [0.5, 0.1, 0.9], [0.0, 1.0, 0.4], [0.7, 0.7, 0.2], [1.0, 0.0, 0.6]], np.float32)
+    cvs = [0.0, 0.25, 0.5, 0.75, 1.0, 0.125, 0.875, -3.0, 7.0, 0.3]
+    w = mk([(0, 0, 0, 0.1, 1, v) for v in cvs], c, lut_e=lut, brightness=(2.0,))
+    tab, ok = oracle.splat_table(w)
+    assert ok.all()
+    E = tab[:, 5:8]
+    L = lut.astype(np.float64)
+    for k in range(5):
+        np.testing.assert_array_equal(E[k], 2.0 * L[k])                      # nodes return table entries
+    np.testing.assert_allclose(E[5], 2.0 * 0.5 * (L[0] + L[1]), rtol=1e-15)   # midpoints return averages
+    np.testing.assert_allclose(E[6], 2.0 * 0.5 * (L[3] + L[4]), rtol=1e-15)
+    np.testing.assert_array_equal(E[7], 2.0 * L[0])                           # clamp below / above
+    np.testing.assert_array_equal(E[8], 2.0 * L[4])
+    u = float(np.float32(0.3)) * 4
+    np.testing.assert_allclose(E[9], 2.0 * ((2 - u) * L[1] + (u - 1) * L[2]), rtol=1e-14)
+    np.testing.assert_array_equal(tab[:, 8:11], E)                            # additive: A == E
+
+
+# P12: equal fp32 depth keys composite in particle-index order, lower index in front (R11)
+def test_p12_tie_order_by_index():
+    c = cam(eye=(0, 0, -10.0), fov=10.0, w=16, h=16)
+    a = (0.0, 0.0, 0.0, 0.3, 2.0, 0.0)
+    b = (0.0, 0.0, 0.0, 0.3, 2.0, 1.0)
+    kw = dict(lut_e=_LUT2E, lut_a=_LUT2A, mode=ABSORB)
+    o_ab = oracle.render(mk([a, b], c, **kw))
+    o_ba = oracle.render(mk([b, a], c, **kw))
+    assert np.abs(o_ab - o_ba).max() > 1e-2
+    # expected: index 0 in front, i.e. C = C_0 + T_0 C_1 at the centre pixel region
+    tab, _ = oracle.splat_table(mk([a, b], c, **kw))
+    jj, ii = np.meshgrid(np.arange(16) + 0.5, np.arange(16) + 0.5, indexing="ij")
+    d2 = (ii - tab[0, 0]) ** 2 + (jj - tab[0, 1]) ** 2
+    tau = np.where(d2 <= tab[0, 3] ** 2, tab[0, 4] * np.exp(-d2 / tab[0, 2] ** 2), 0.0)[:, :, None]
+    E0, A0, E1, A1 = (_LUT2E[0].astype(np.float64), _LUT2A[0].astype(np.float64),
+                      _LUT2E[1].astype(np.float64), _LUT2A[1].astype(np.float64))
+
+    def contrib(E, A):
+        u = A * tau
+        return E * tau * np.where(u > 0, -np.expm1(-u) / np.where(u > 0, u, 1), 1.0), np.exp(-u)
+
+    c0, t0 = contrib(E0, A0)
+    c1, t1 = contrib(E1, A1)
+    np.testing.assert_allclose(o_ab, c0 + t0 * c1, rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(o_ba, c1 + t1 * c0, rtol=1e-12, atol=1e-15)
+
+
+def test_absorb_zero_absorption_channel_is_pure_emission():
+    """R15: A_c = 0 gives phi = 1, i.e. the channel accumulates E tau like raw additive S."""
+    c = cam(eye=(0, 0, -10.0), fov=10.0, w=16, h=16)
+    pts = [(0.0, 0.0, 0.0, 0.3, 2.0, 0.0), (0.1, 0.05, 1.0, 0.2, 1.0, 1.0)]
+    lut_a = np.array([[0.0, 0.4, 0.0], [0.0, 0.9, 0.0]], np.float32)
+    out = oracle.render(mk(pts, c, lut_e=_LUT2E, lut_a=lut_a, mode=ABSORB))
+    raw = oracle.render(mk(pts, c, lut_e=_LUT2E), raw=True)
+    np.testing.assert_allclose(out[:, :, 0], raw[:, :, 0], rtol=1e-13)
+    np.testing.assert_allclose(out[:, :, 2], raw[:, :, 2], rtol=1e-13)
+    assert np.all(out[:, :, 1] <= raw[:, :, 1] + 1e-15) and np.abs(out[:, :, 1] - raw[:, :, 1]).max() > 1e-3
