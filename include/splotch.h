@@ -1,0 +1,215 @@
+/*
+ * splotch.h -- C ABI of the B200-native Splotch render hot path.
+ *
+ * What the library computes (arxiv 1004.1302, "High-performance astrophysical visualization
+ * using Splotch"; citations are lines of /root/reference/PAPER.md):
+ *
+ *   - every particle is a Gaussian blob rho_p(r) = rho_0p exp(-r^2/sigma_p^2), set to zero
+ *     beyond f*sigma_p; a ray farther than f*sigma_p from it is unaffected
+ *   - R, G, B are three independent "frequencies"
+ *   - along a ray  dI/dx = (E_p - A_p I) rho_p(x)                          (Eq. 1)
+ *   - E_p, A_p come from a scalar through a colour look-up table; the optical depth can be
+ *     modulated by another scalar; E_p = A_p is the recommended setting
+ *   - "displaying involves transformation into screen coordinates, assigning of colours and
+ *     rendering for determining screen areas affected by individual particles and
+ *     subsequently combining them for final imaging"
+ *
+ * The readings of everything the paper leaves open (camera model, image orientation, point
+ * sampling at pixel centres, rho_0 = I, sigma = r, truncation by impact parameter, slab
+ * compositing in depth order when A != E, tie order) are listed in DESIGN.md "Readings".
+ *
+ * Conventions
+ *   - All array arguments of splotch_render / splotch_debug_* are DEVICE pointers unless the
+ *     name says host.  Structs themselves are host memory, passed by pointer, read during
+ *     the call only.
+ *   - Ownership: every buffer is caller-owned.  The library never allocates or frees device
+ *     memory and keeps no pointer after a call returns.  Particle arrays and colour tables
+ *     are read-only.  `out_rgb` is overwritten.  The workspace content is undefined after a
+ *     call except for its status head (splotch_workspace_status).
+ *   - Asynchrony: splotch_render, splotch_normalize and the debug calls only enqueue work on
+ *     `stream` (a cudaStream_t passed as void*, NULL = default stream) and return without
+ *     synchronising.  Calls whose name ends in _sync or that return host values synchronise
+ *     the stream; they say so below.
+ *   - Image layout: out_rgb[(row * width + col) * 3 + c], float32, row 0 = top of the image,
+ *     c = 0,1,2 = R,G,B.  Pixel (col i, row j) is sampled at its centre (i + 1/2, j + 1/2).
+ *   - Errors: 0 = SPLOTCH_OK, negative = error, nothing is ever reported through the image.
+ *     Particles with a non-finite field, r <= 0, type >= n_types, behind the near plane or
+ *     covering no pixel centre are culled silently; they are not errors.
+ *   - No CPU fallback exists: without a CUDA device every compute entry point returns
+ *     SPLOTCH_ERR_CUDA.
+ */
+#ifndef SPLOTCH_H
+#define SPLOTCH_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPLOTCH_MAX_TYPES 4
+
+/* status codes */
+#define SPLOTCH_OK 0
+#define SPLOTCH_ERR_INVALID_ARG (-1) /* NULL required pointer, n < 0, bad camera, bad params    */
+#define SPLOTCH_ERR_WORKSPACE (-2)   /* workspace_bytes too small, or pair count > max_pairs    */
+#define SPLOTCH_ERR_CUDA (-3)        /* a CUDA call failed; see splotch_last_cuda_error()        */
+#define SPLOTCH_ERR_LIMIT (-4)       /* a size exceeds what the library supports (see below)    */
+
+/* Limits: n < 2^31; width, height <= 16384; n_entries >= 2; n_types in 1..SPLOTCH_MAX_TYPES;
+ * max_pairs < 2^32. */
+
+/* Particle arrays, structure-of-arrays as in the paper's files ("x coordinates of all
+ * particles, then y coordinates and so on").  Length n each. */
+typedef struct {
+    const float *x, *y, *z;   /* world position                                               */
+    const float *r;           /* smoothing length = sigma_p of PAPER.md:69                    */
+    const float *I;           /* optical-depth modulation = rho_0p (last sentence) */
+    const float *colval;      /* scalar mapped through the colour table, clamped to [0, 1]    */
+    const uint8_t *type;      /* particle type 0..n_types-1; NULL means all type 0            */
+} splotch_particles;
+
+/* Pinhole perspective camera (reading R1, R2): fwd = normalise(lookat - eye),
+ * right = normalise(fwd x up), upv = right x fwd, focal length F = (width/2) / tan(fov/2)
+ * pixels, fov the full horizontal angle in degrees, 0 < fov < 180. */
+typedef struct {
+    float eye[3], lookat[3], up[3];
+    float fov_deg;
+    int32_t width, height;
+} splotch_camera;
+
+/* Colour look-up tables: n_types * n_entries * 3 floats, RGB interleaved, type
+ * major.  Sampled piece-wise linearly between n_entries equally spaced nodes on [0, 1]. */
+typedef struct {
+    const float *emission;    /* E table                                                      */
+    const float *absorption;  /* A table; ignored (may be NULL) in additive mode              */
+    int32_t n_entries, n_types;
+} splotch_colormap;
+
+typedef enum { SPLOTCH_ADDITIVE = 0, SPLOTCH_ABSORB = 1 } splotch_mode;
+
+#define SPLOTCH_RAW_SUM 1u /* additive mode writes S_c = sum_p E_pc tau_p, not 1 - exp(-S_c)   */
+
+typedef struct {
+    float brightness[SPLOTCH_MAX_TYPES];     /* scales E per type                             */
+    float abs_brightness[SPLOTCH_MAX_TYPES]; /* scales A per type (absorb mode)               */
+    int32_t mode;                            /* splotch_mode                                  */
+    float support_f;                         /* f of PAPER.md:69; > 0; the configs use 3      */
+    float z_near;                            /* cull view-space depth <= z_near               */
+    uint32_t flags;                          /* SPLOTCH_RAW_SUM                               */
+} splotch_params;
+
+/* ------------------------------------------------------------------------------------------
+ * The render call.
+ *
+ * SPLOTCH_ADDITIVE (A_p = E_p): out_c = 1 - exp(-S_c), S_c = sum over particles of
+ *   E_pc * I_p r_p sqrt(pi) * exp(-d^2 / sigma_s^2) for pixels with d^2 <= (f sigma_s)^2, the
+ *   exact solution of Eq. (1) when absorption equals emission; any summation order.
+ * SPLOTCH_ABSORB (A_p != E_p): particles composited front to back in order of ascending
+ *   (fp32 view depth, particle index):  C_c += T_c E_pc tau phi(A_pc tau),  T_c *= exp(-A_pc tau),
+ *   phi(u) = (1 - exp(-u))/u; out_c = C_c.  This is Eq. (1) integrated across one particle
+ *   at a time (slab reading R10).
+ *
+ * workspace: device memory, >= splotch_workspace_bytes(...) bytes, 256-byte aligned.
+ * max_pairs: capacity of the (particle, 64x64-pixel block) pair list; use
+ *   splotch_count_pairs() or an upper bound.  If the scene needs more, the image is
+ *   zero-filled and SPLOTCH_ERR_WORKSPACE is recorded in the workspace status head.
+ * Returns after enqueueing on `stream`; does not synchronise.
+ * ---------------------------------------------------------------------------------------- */
+int splotch_workspace_bytes(int64_t n, const splotch_camera *camera, const splotch_params *params,
+                            uint64_t max_pairs, uint64_t *bytes);
+
+int splotch_render(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                   const splotch_colormap *colormap, const splotch_params *params, float *out_rgb,
+                   void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream);
+
+/* Reads the status head the last call left in `workspace`.  SYNCHRONISES `stream`.
+ * status: SPLOTCH_OK or SPLOTCH_ERR_WORKSPACE; visible: particles that passed culling;
+ * pairs: (particle, block) pairs the scene needs.  Any output pointer may be NULL. */
+int splotch_workspace_status(const void *workspace, void *stream, int32_t *status, uint64_t *visible,
+                             uint64_t *pairs);
+
+/* Runs the transform / cull / bin-count steps only and returns the pair count and the
+ * visible count to the host.  SYNCHRONISES `stream`.  workspace must be at least
+ * splotch_workspace_bytes(n, camera, params, 0, ...) bytes. */
+int splotch_count_pairs(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                        const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                        uint64_t workspace_bytes, uint64_t *pairs_host, uint64_t *visible_host, void *stream);
+
+/* out[k] = 1 - exp(-S[k]) for k < n_values (the additive output map, reading R13); S may
+ * equal out.  Exposed for the multi-GPU path, which sums raw S images before this step. */
+int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream);
+
+/* End-to-end variant with HOST buffers: copies the particle arrays and colour tables to the
+ * device (staging areas inside `workspace`), renders, copies the image back to
+ * `out_rgb_host` and SYNCHRONISES.  All pointers inside `particles_host` and
+ * `colormap_host` and `out_rgb_host` are host pointers (pinned memory gives the best copy
+ * rate).  workspace must be at least splotch_workspace_bytes_host(...) bytes of device memory. */
+int splotch_workspace_bytes_host(int64_t n, const splotch_camera *camera, const splotch_colormap *colormap_host,
+                                 const splotch_params *params, uint64_t max_pairs, uint64_t *bytes);
+
+int splotch_render_host(const splotch_particles *particles_host, int64_t n, const splotch_camera *camera,
+                        const splotch_colormap *colormap_host, const splotch_params *params,
+                        float *out_rgb_host, void *workspace, uint64_t workspace_bytes, uint64_t max_pairs,
+                        void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Test-only exports for the bit-exact checks (north_star: "Tile/bin indices and counts must be
+ * bit-exact").  They run the SAME kernels as splotch_render with extra outputs.
+ *
+ * splotch_debug_project: per particle (device arrays of length n; any may be NULL)
+ *   sx, sy     screen position in pixels;  sigma_s = F r / z_c;  R = f sigma_s
+ *   zkey       bit pattern of the fp32 view depth z_c (the depth key, R11)
+ *   pix_bbox   n*4 int32: i0, i1, j0, j1, inclusive box of candidate pixels
+ *   visible    1 if the particle passed culling, else 0 (all other outputs 0)
+ *
+ * splotch_debug_bins: bins of 2^bin_shift x 2^bin_shift pixels (4 = the 16x16 tiles of
+ *   north_star, 6 = the 64x64 blocks the rasteriser consumes).  A visible particle belongs to
+ *   every bin its pixel box touches; bin index = by * ceil(width / 2^bin_shift) + bx.
+ *   tile_count   T uint32;  tile_offset  T+1 uint64 (exclusive prefix sum, last = D)
+ *   member_ids   D uint32 particle indices, bin by bin (may be NULL).  Additive mode: order
+ *                inside a bin is unspecified.  Absorb mode: ascending (zkey, index).
+ *   max_members  capacity of member_ids; if D exceeds it member_ids is left untouched.
+ *   Limits: width, height <= 256 * 2^bin_shift.
+ *
+ * splotch_debug_stats (SYNCHRONISES): host outputs: visible count, pair count at
+ *   `bin_shift`, and the exact number of (particle, covered pixel) updates U.
+ * ---------------------------------------------------------------------------------------- */
+int splotch_debug_project(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                          const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                          uint64_t workspace_bytes, float *sx, float *sy, float *sigma_s, float *R,
+                          uint32_t *zkey, int32_t *pix_bbox, uint8_t *visible, void *stream);
+
+int splotch_debug_bins(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                       const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                       uint64_t workspace_bytes, int32_t bin_shift, uint32_t *tile_count,
+                       uint64_t *tile_offset, uint32_t *member_ids, uint64_t max_members, void *stream);
+
+int splotch_debug_workspace_bytes(int64_t n, const splotch_camera *camera, const splotch_params *params,
+                                  int32_t bin_shift, uint64_t max_members, uint64_t *bytes);
+
+int splotch_debug_stats(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                        const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                        uint64_t workspace_bytes, int32_t bin_shift, uint64_t *visible_host,
+                        uint64_t *pairs_host, uint64_t *updates_host, void *stream);
+
+/* Device-wide building blocks, exported so that tests can check them in isolation.
+ * splotch_debug_scan: out[k] = sum_{m<k} in[k] for k <= n (n+1 outputs, 64-bit), the
+ *   single-pass decoupled look-back scan used for bin offsets.  scratch: >= (n/2048 + 2) * 8 + 256 bytes.
+ * splotch_debug_sort_pairs: stable LSD radix sort of (key, value) uint32 pairs on key bits
+ *   [0, key_bits); keys_tmp / vals_tmp are ping-pong buffers of length n; the sorted result
+ *   ends in (keys, vals).  scratch: >= splotch_sort_scratch_bytes(n). */
+int splotch_debug_scan(const uint32_t *in, uint64_t *out, int64_t n, void *scratch, uint64_t scratch_bytes,
+                       void *stream);
+uint64_t splotch_sort_scratch_bytes(int64_t n);
+int splotch_debug_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
+                             int32_t key_bits, void *scratch, uint64_t scratch_bytes, void *stream);
+
+const char *splotch_status_string(int status);
+int splotch_last_cuda_error(void);  /* cudaError_t of the last failing CUDA call in this thread */
+int splotch_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPLOTCH_H */

@@ -84,8 +84,8 @@ static int finite6(float a, float b, float c, float d, float e, float f)
 /* ---------------------------------------------------------------------------------------
  * Canonical fp32 projector (SURVEY.md 8(c) "Canonical fp32 sequence", DESIGN.md "Canonical
  * sequence").  Every operation is one correctly rounded binary32 operation.
- *   visible[p] = 1 iff all six fields finite, r > 0, type < n_types, zc > z_near, ss > 0
- *                and the pixel box is non-empty.
+ *   visible[p] = 1 iff all six fields finite, r > 0, type < n_types, zc > z_near, ss > 0,
+ *                R finite and the pixel box is non-empty.
  *   bbox[4p..] = i0, i1, j0, j1 (inclusive pixel box; column i, row j; row 0 = top)
  *   zkey[p]    = bit pattern of zc (positive floats order as unsigned integers), R11.
  * Outputs for culled particles: visible 0, everything else 0.
@@ -122,7 +122,7 @@ int orc_project_f32(int64_t n, const float *x, const float *y, const float *z, c
         float psy = fmaf(-yc, q, cy);
         float pss = r[p] * q;
         float pR = support_f * pss;
-        if (!(pss > 0.0f)) continue;
+        if (!(pss > 0.0f) || !isfinite(pR)) continue;   /* degenerate footprint: culled (R6) */
         /* pixel (i, j) has its centre at (i + 1/2, j + 1/2): covered candidates satisfy
            sx - R <= i + 1/2 <= sx + R */
         float i0f = fminf(fmaxf(ceilf((psx - pR) - 0.5f), 0.0f), Wf);

@@ -1,0 +1,165 @@
+// common.cuh -- shared declarations of the sm_100a Splotch render library (product code).
+// Nothing here is shared with oracle/ (the CPU oracle is an independent restatement).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace splotch {
+
+// ---------------------------------------------------------------------------------------------
+// geometry of the rasteriser: one CTA owns a 64x64-pixel block, one warp a 16x16 tile of it,
+// one lane a strip of 8 consecutive pixels of one tile row.
+// ---------------------------------------------------------------------------------------------
+constexpr int kBlockShift = 6;             // production bins: 64x64 pixels
+constexpr int kBlockPx = 1 << kBlockShift;
+constexpr int kTilePx = 16;
+constexpr int kMaxBinsPerAxis = 256;       // packed 8-bit bin coordinates in the splat record
+constexpr int kMaxImage = 16384;
+
+// ---------------------------------------------------------------------------------------------
+// camera constants, computed on the host in double and rounded once to fp32 (DESIGN.md
+// "Canonical sequence"); passed to kernels by value.
+// ---------------------------------------------------------------------------------------------
+struct CameraConst {
+    float ex, ey, ez;
+    float rx, ry, rz;      // right
+    float ux, uy, uz;      // upv
+    float fx, fy, fz;      // fwd
+    float F, cx, cy;       // focal length in pixels, W/2, H/2
+    float Wf, Hf;
+    int W, H;
+};
+
+struct RenderConst {
+    float brightness[4];
+    float abs_brightness[4];
+    float support_f;
+    float z_near;
+    float thr;             // exp(-f^2): coverage threshold on the Gaussian weight
+    int n_entries, n_types;
+    int mode;              // 0 additive, 1 absorb
+    int bin_shift;         // bins of 2^bin_shift pixels
+    int nbx, nby;          // bins per axis
+};
+
+// ---------------------------------------------------------------------------------------------
+// splat records written by the transform / cull / colour kernel (step a1-a3)
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t kInvisible = 0xFFFFFFFFu;
+
+struct __align__(16) SplatAdd {     // 32 B, additive mode
+    float sx, sy;                   // screen position (pixels)
+    float c;                        // sqrt(log2 e) / sigma_s : weight = exp2(-((d * c)^2))
+    float R;                        // f * sigma_s
+    float ar, ag, ab;               // a_c = E_c * I * r * sqrt(pi)
+    uint32_t bins;                  // bx0 | bx1 << 8 | by0 << 16 | by1 << 24, or kInvisible
+};
+
+struct __align__(16) SplatAbs {     // 48 B, absorb mode
+    float sx, sy, c, R;
+    float tau0;                     // I * r * sqrt(pi)
+    float Er, Eg, Eb;
+    float Ar, Ag, Ab;
+    uint32_t bins;
+};
+
+// record field access shared by the binning kernels: the packed bin box is the last word
+__device__ __forceinline__ uint32_t record_bins(const void *records, int record_bytes, long long i)
+{
+    return __ldg(reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(records) +
+                                                    (size_t)i * record_bytes + record_bytes - 4));
+}
+
+// device-side status head at the start of every workspace (256 B reserved)
+struct WorkHead {
+    int32_t status;                 // SPLOTCH_OK or SPLOTCH_ERR_WORKSPACE
+    uint32_t n_units;               // raster work units
+    unsigned long long visible;     // particles that passed culling
+    unsigned long long pairs;       // (particle, bin) pairs
+    unsigned long long updates;     // debug_stats: (particle, covered pixel) updates
+    uint32_t work_counter;          // persistent-kernel ticket
+    uint32_t scan_ticket;           // decoupled look-back tile ticket
+    uint32_t pad[6];
+};
+
+// ---------------------------------------------------------------------------------------------
+// error plumbing
+// ---------------------------------------------------------------------------------------------
+extern thread_local int g_last_cuda_error;
+
+#define SPLOTCH_CUDA_TRY(expr)                                   \
+    do {                                                         \
+        cudaError_t e__ = (expr);                                \
+        if (e__ != cudaSuccess) {                                \
+            ::splotch::g_last_cuda_error = (int)e__;             \
+            return -3; /* SPLOTCH_ERR_CUDA */                    \
+        }                                                        \
+    } while (0)
+
+#define SPLOTCH_LAUNCH_CHECK() SPLOTCH_CUDA_TRY(cudaGetLastError())
+
+inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+int sm_count();
+
+// ---------------------------------------------------------------------------------------------
+// launchers (each only enqueues on `st`)
+// ---------------------------------------------------------------------------------------------
+struct ParticlePtrs {
+    const float *x, *y, *z, *r, *I, *colval;
+    const uint8_t *type;
+};
+
+struct DebugProjectOut {
+    float *sx, *sy, *sigma_s, *R;
+    uint32_t *zkey;
+    int32_t *pix_bbox;
+    uint8_t *visible;
+};
+
+// scan.cu: out[k] = sum_{m<k} in[m], k = 0..n (n+1 outputs)
+uint64_t scan_scratch_bytes(int64_t n);
+int launch_scan_u32_u64(const uint32_t *in, uint64_t *out, int64_t n, void *scratch, cudaStream_t st);
+int launch_scan_u32_u32(const uint32_t *in, uint32_t *out, int64_t n, void *scratch, cudaStream_t st);
+
+// sort.cu
+uint64_t sort_scratch_bytes(int64_t n);
+int launch_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
+                      const unsigned long long *n_dev, int key_bits, void *scratch, cudaStream_t st,
+                      bool *result_in_tmp);
+
+// project.cu (K1): records + fused bin counts (+ optional debug outputs, + depth keys in absorb mode)
+int launch_project(const ParticlePtrs &p, int64_t n, const CameraConst &cam, const RenderConst &rc,
+                   const float *lutE, const float *lutA, void *records, uint32_t *bin_count, uint32_t *zkeys,
+                   WorkHead *head, const DebugProjectOut *dbg, cudaStream_t st);
+
+// bin.cu (K2)
+int launch_finish_offsets(const uint32_t *bin_count, const uint64_t *bin_offset, int n_bins, uint64_t max_pairs,
+                          uint32_t chunk, uint32_t *unit_prefix, WorkHead *head, cudaStream_t st);
+int launch_scatter(const void *records, int record_bytes, int64_t n, const RenderConst &rc,
+                   const uint64_t *bin_offset, uint32_t *bin_cursor, uint32_t *list, uint64_t max_pairs,
+                   const WorkHead *head, cudaStream_t st);
+int launch_count_updates(const void *records, int record_bytes, int64_t n, const CameraConst &cam, float thr,
+                         WorkHead *head, cudaStream_t st);
+// absorb: pair expansion in depth order
+int launch_pair_counts(const void *records, int record_bytes, const uint32_t *sorted_ids, int64_t n,
+                       uint32_t *pair_count, cudaStream_t st);
+int launch_expand_pairs(const void *records, int record_bytes, const uint32_t *sorted_ids, int64_t n,
+                        const uint64_t *pair_offset, const RenderConst &rc, uint32_t *pair_bin, uint32_t *pair_id,
+                        uint64_t max_pairs, const WorkHead *head, cudaStream_t st);
+int launch_iota(uint32_t *v, int64_t n, cudaStream_t st);
+
+// raster.cu (K3, K4)
+constexpr uint32_t kChunkAdd = 2048;   // splats per additive work unit
+constexpr uint32_t kChunkAbs = 4096;   // splats per absorb work unit
+int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
+                           const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
+                           WorkHead *head, cudaStream_t st);
+int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const uint64_t *bin_offset,
+                         const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam,
+                         float *partials, WorkHead *head, cudaStream_t st);
+int launch_merge_absorb(const float *partials, const uint32_t *unit_prefix, const RenderConst &rc,
+                        const CameraConst &cam, float *out, const WorkHead *head, cudaStream_t st);
+int launch_normalize(const float *S, float *out, int64_t n_values, cudaStream_t st);
+
+}  // namespace splotch

@@ -1,0 +1,154 @@
+"""Convenience layer over the binding: device residency of a particle set and one-call renders.
+
+Argument marshalling and memory management only (PyTorch owns device memory and streams);
+every step of the path runs in libsplotch_b200.so.
+"""
+from __future__ import annotations
+
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+
+def _camera_struct(cam) -> B.splotch_camera:
+    return B.make_camera(cam.eye, cam.lookat, cam.up, cam.fov_deg, cam.width, cam.height)
+
+
+class Scene:
+    """A particle set resident in HBM plus its colour tables and parameters.
+
+    `w` is any object with the fields of workloads.Workload (numpy arrays x, y, z, r, I, colval,
+    optional uint8 type, lut_e/lut_a of shape (n_types, n_entries, 3), brightness lists, mode,
+    support_f, z_near, cameras)."""
+
+    def __init__(self, w, device: str = "cuda:0", resident: bool = True):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1004_1302_b200 needs a CUDA device: there is no CPU fallback")
+        B.library_path()   # fail loudly if the extension is missing
+        self.device = torch.device(device)
+        self.w = w
+        self.n = int(w.n)
+        self.n_types, self.n_entries = int(w.lut_e.shape[0]), int(w.lut_e.shape[1])
+        self._host = {k: np.ascontiguousarray(getattr(w, k), np.float32) for k in ("x", "y", "z", "r", "I", "colval")}
+        self._host_type = None if w.type is None else np.ascontiguousarray(w.type, np.uint8)
+        self._host_lut_e = np.ascontiguousarray(w.lut_e, np.float32)
+        self._host_lut_a = None if w.lut_a is None else np.ascontiguousarray(w.lut_a, np.float32)
+        self.d = {}
+        self.workspace: Optional[torch.Tensor] = None
+        self.max_pairs = 0
+        if resident:
+            self.upload()
+
+    # ---- device residency ----------------------------------------------------------------
+    def upload(self) -> None:
+        with torch.cuda.device(self.device):
+            for k, a in self._host.items():
+                self.d[k] = torch.from_numpy(a).to(self.device)
+            self.d["type"] = None if self._host_type is None else torch.from_numpy(self._host_type).to(self.device)
+            self.d["lut_e"] = torch.from_numpy(self._host_lut_e).to(self.device)
+            self.d["lut_a"] = None if self._host_lut_a is None else torch.from_numpy(self._host_lut_a).to(self.device)
+            torch.cuda.synchronize(self.device)
+
+    def particles(self) -> B.splotch_particles:
+        d = self.d
+        return B.make_particles(d["x"], d["y"], d["z"], d["r"], d["I"], d["colval"], d["type"])
+
+    def colormap(self) -> B.splotch_colormap:
+        return B.make_colormap(self.d["lut_e"], self.d["lut_a"], self.n_entries, self.n_types)
+
+    def params(self, mode: Optional[int] = None, raw: bool = False) -> B.splotch_params:
+        w = self.w
+        return B.make_params(w.brightness, w.abs_brightness, w.mode if mode is None else mode, w.support_f, w.z_near,
+                             B.SPLOTCH_RAW_SUM if raw else 0)
+
+    def _alloc(self, nbytes: int) -> torch.Tensor:
+        return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=self.device)
+
+    @staticmethod
+    def _aligned(t: torch.Tensor) -> int:
+        return (t.data_ptr() + 255) // 256 * 256
+
+    # ---- sizing ---------------------------------------------------------------------------
+    def count_pairs(self, cam=None, mode: Optional[int] = None):
+        """(pairs, visible) for a camera; synchronises."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(mode)
+        nbytes = B.splotch_workspace_bytes(self.n, cs, ps, 0)
+        ws = self._alloc(nbytes)
+        return B.splotch_count_pairs(self.particles(), self.n, cs, self.colormap(), ps, self._aligned(ws), nbytes)
+
+    def reserve(self, cam=None, mode: Optional[int] = None, max_pairs: Optional[int] = None, slack: float = 1.02) -> int:
+        """Size and allocate the workspace for `cam` (or for an explicit max_pairs)."""
+        cam = cam or self.w.camera
+        if max_pairs is None:
+            pairs, _ = self.count_pairs(cam, mode)
+            max_pairs = int(pairs * slack) + 1024
+        cs, ps = _camera_struct(cam), self.params(mode)
+        nbytes = B.splotch_workspace_bytes(self.n, cs, ps, max_pairs)
+        if self.workspace is None or self.workspace.numel() < nbytes + 256:
+            self.workspace = None
+            self.workspace = self._alloc(nbytes)
+        self.max_pairs = int(max_pairs)
+        return nbytes
+
+    # ---- the render call ------------------------------------------------------------------
+    def render(self, cam=None, mode: Optional[int] = None, raw: bool = False, out: Optional[torch.Tensor] = None,
+               check: bool = True) -> torch.Tensor:
+        """One splotch_render on the current stream.  Returns a float32 (H, W, 3) CUDA tensor."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(mode, raw)
+        nbytes = B.splotch_workspace_bytes(self.n, cs, ps, self.max_pairs) if self.workspace is not None else None
+        if self.workspace is None or self.workspace.numel() < nbytes + 256:
+            nbytes = self.reserve(cam, mode)
+        if out is None:
+            out = torch.empty((cam.height, cam.width, 3), dtype=torch.float32, device=self.device)
+        B.splotch_render(self.particles(), self.n, cs, self.colormap(), ps, out, self._aligned(self.workspace),
+                         self.workspace.numel() - 256, self.max_pairs)
+        if check:
+            status, _, pairs = B.splotch_workspace_status(self._aligned(self.workspace))
+            if status != B.SPLOTCH_OK:
+                raise B.SplotchError(f"splotch_render (scene needs {pairs} pairs, max_pairs={self.max_pairs})", status)
+        return out
+
+    def stats(self, cam=None, mode: Optional[int] = None, bin_shift: int = 6):
+        """(visible, pairs at bin_shift, pixel updates U); synchronises."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(mode)
+        nbytes = B.splotch_debug_workspace_bytes(self.n, cs, ps, bin_shift, 0)
+        ws = self._alloc(nbytes)
+        return B.splotch_debug_stats(self.particles(), self.n, cs, self.colormap(), ps, self._aligned(ws), nbytes, bin_shift)
+
+    # ---- end to end with host buffers ---------------------------------------------------------
+    def host_buffers(self, pinned: bool = True):
+        """Pinned host copies of the inputs and a pinned output image for render_host."""
+        def pin(a):
+            t = torch.from_numpy(a)
+            return t.pin_memory() if pinned else t
+        hb = {k: pin(a) for k, a in self._host.items()}
+        hb["type"] = None if self._host_type is None else pin(self._host_type)
+        hb["lut_e"] = pin(self._host_lut_e)
+        hb["lut_a"] = None if self._host_lut_a is None else pin(self._host_lut_a)
+        return hb
+
+    def render_host(self, hb, cam=None, mode: Optional[int] = None, out_host: Optional[torch.Tensor] = None,
+                    max_pairs: Optional[int] = None, workspace: Optional[torch.Tensor] = None):
+        """splotch_render_host: H2D copies + render + D2H copy + sync inside the library call."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(mode)
+        max_pairs = self.max_pairs if max_pairs is None else max_pairs
+        ph = B.make_particles(hb["x"], hb["y"], hb["z"], hb["r"], hb["I"], hb["colval"], hb["type"])
+        cmh = B.make_colormap(hb["lut_e"], hb["lut_a"], self.n_entries, self.n_types)
+        nbytes = B.splotch_workspace_bytes_host(self.n, cs, cmh, ps, max_pairs)
+        if workspace is None:
+            workspace = self._alloc(nbytes)
+        if out_host is None:
+            out_host = torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory()
+        B.splotch_render_host(ph, self.n, cs, cmh, ps, out_host, self._aligned(workspace), nbytes, max_pairs)
+        return out_host, workspace
+
+    def h2d_bytes(self) -> int:
+        lut = self._host_lut_e.nbytes + (0 if self._host_lut_a is None else self._host_lut_a.nbytes)
+        return self.n * (24 + (0 if self._host_type is None else 1)) + lut

@@ -1,0 +1,357 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): integers (visible set, pixel boxes, depth keys, bin counts,
+offsets, membership) bit-exact; pixels within |delta| <= 1e-4 * max(1, |ref|) in both modes.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from workloads import ABSORB, ADDITIVE
+
+from helpers import cam, const_lut, mk
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1004_1302_b200 import binding
+    binding.library_path()
+    return binding
+
+
+def _scene(w):
+    from paper_1004_1302_b200 import Scene
+    return Scene(w)
+
+
+def _tol_check(out, ref, what=""):
+    out = np.asarray(out, np.float64)
+    err = np.abs(out - ref)
+    bound = 1e-4 * np.maximum(1.0, np.abs(ref))
+    worst = float((err / bound).max()) if err.size else 0.0
+    assert worst <= 1.0, f"{what}: worst |delta| / (1e-4 max(1,|ref|)) = {worst:.3f} at {np.unravel_index((err / bound).argmax(), err.shape)}"
+    return worst
+
+
+# ------------------------------------------------------------------------------------------------
+# building blocks
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [0, 1, 5, 2047, 2048, 2049, 70_001, 1_000_003])
+def test_scan_matches_cumsum(B, n):
+    rs = np.random.RandomState(n % 1000)
+    a = rs.randint(0, 2 ** 32, size=max(n, 1), dtype=np.uint64).astype(np.uint32)[:n]
+    d_in = torch.from_numpy(a.astype(np.int64)).to("cuda").to(torch.int64)
+    d_in32 = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
+    if n:
+        d_in32[:n] = torch.from_numpy(a.view(np.int32)).cuda()
+    out = torch.zeros(n + 1, dtype=torch.int64, device="cuda")
+    sb = (n // 2048 + 2) * 8 + 512
+    scratch = torch.empty(sb, dtype=torch.uint8, device="cuda")
+    B.splotch_debug_scan(d_in32, out, n, scratch, sb)
+    torch.cuda.synchronize()
+    expect = np.concatenate([[0], np.cumsum(a.astype(np.uint64))]).astype(np.uint64)
+    np.testing.assert_array_equal(out.cpu().numpy().view(np.uint64), expect)
+
+
+@pytest.mark.parametrize("n,bits", [(1, 8), (31, 8), (4095, 12), (4096, 32), (4097, 32), (300_001, 32), (1_000_000, 10)])
+def test_radix_sort_is_stable_and_sorted(B, n, bits):
+    rs = np.random.RandomState(bits * 7 + n % 13)
+    keys = rs.randint(0, 2 ** min(bits, 31), size=n, dtype=np.int64).astype(np.uint32)
+    if bits == 32:
+        keys |= (rs.randint(0, 2, size=n).astype(np.uint32) << np.uint32(31))
+    keys[: n // 3] = keys[: n // 3] & np.uint32(0xFF)                        # many ties
+    vals = np.arange(n, dtype=np.uint32)
+    dk = torch.from_numpy(keys.view(np.int32)).cuda()
+    dv = torch.from_numpy(vals.view(np.int32)).cuda()
+    tk, tv = torch.empty_like(dk), torch.empty_like(dv)
+    sb = B.splotch_sort_scratch_bytes(n)
+    scratch = torch.empty(sb, dtype=torch.uint8, device="cuda")
+    B.splotch_debug_sort_pairs(dk, dv, tk, tv, n, bits, scratch, sb)
+    torch.cuda.synchronize()
+    order = np.argsort(keys, kind="stable")
+    np.testing.assert_array_equal(dv.cpu().numpy().view(np.uint32), order.astype(np.uint32))
+    np.testing.assert_array_equal(dk.cpu().numpy().view(np.uint32), keys[order])
+
+
+# ------------------------------------------------------------------------------------------------
+# K1: bit-exact projection, culling, depth key
+# ------------------------------------------------------------------------------------------------
+def _gpu_project(B, w, camera=None):
+    sc = _scene(w)
+    camera = camera or w.camera
+    n = w.n
+    from paper_1004_1302_b200.scene import _camera_struct
+    cs, ps = _camera_struct(camera), sc.params()
+    nbytes = B.splotch_debug_workspace_bytes(n, cs, ps, 6, 0)
+    ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    o = dict(sx=torch.zeros(n, dtype=torch.float32, device="cuda"), sy=torch.zeros(n, dtype=torch.float32, device="cuda"),
+             ss=torch.zeros(n, dtype=torch.float32, device="cuda"), R=torch.zeros(n, dtype=torch.float32, device="cuda"),
+             zkey=torch.zeros(n, dtype=torch.int32, device="cuda"), bbox=torch.zeros((n, 4), dtype=torch.int32, device="cuda"),
+             visible=torch.zeros(n, dtype=torch.uint8, device="cuda"))
+    B.splotch_debug_project(sc.particles(), n, cs, sc.colormap(), ps, sc._aligned(ws), nbytes, o["sx"], o["sy"], o["ss"],
+                            o["R"], o["zkey"], o["bbox"], o["visible"])
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in o.items()}
+    out["zkey"] = out["zkey"].view(np.uint32)
+    return out
+
+
+def _edge_particles():
+    pts = [(0.5, 0.5, 0.5, 0.01, 1.0, 0.5)] * 3
+    pts += [(np.nan, 0.5, 0.5, 0.01, 1, 0), (0.5, np.inf, 0.5, 0.01, 1, 0), (0.5, 0.5, 0.5, -0.01, 1, 0),
+            (0.5, 0.5, 0.5, 0.0, 1, 0), (0.5, 0.5, 0.5, 0.01, np.nan, 0), (0.5, 0.5, 0.5, 0.01, 1, np.inf),
+            (0.5, 0.5, -1.5, 0.01, 1, 0), (0.5, 0.5, -1.4905, 0.01, 1, 0), (0.5, 0.5, -3.0, 0.01, 1, 0),
+            (30.0, 0.5, 0.5, 0.01, 1, 0), (0.5, 0.5, 0.5, 1e-7, 1, 0), (0.5, 0.5, 0.5, 5.0, 1, 0),
+            (0.5, 0.5, 0.5, 1e30, 1, 0), (0.5, 0.5, 0.5, 3e38, 1, 0), (1e30, 0.5, 0.5, 0.01, 1, 0),
+            (0.5, 0.5, 0.5, 1e-38, 1, 0)]
+    return pts
+
+
+@pytest.mark.parametrize("case", ["C1", "C4", "C3", "edge"])
+def test_project_bit_exact(B, case):
+    if case == "C1":
+        w = workloads.make("C1")
+    elif case == "C4":
+        w = workloads.make("C4", 200_003, width=1000, height=700)
+    elif case == "C3":
+        w = workloads.make("C3", 300_001, width=2048, height=2048)
+    else:
+        w = mk(_edge_particles(), workloads.make("C1", 10).camera)
+    ref = oracle.project_f32(w)
+    got = _gpu_project(B, w)
+    np.testing.assert_array_equal(got["visible"], ref["visible"])
+    assert 0 < ref["visible"].sum() < w.n or case == "edge"
+    for k in ("sx", "sy", "ss", "R"):
+        np.testing.assert_array_equal(got[k].view(np.uint32), ref[k].view(np.uint32), err_msg=k)
+    np.testing.assert_array_equal(got["zkey"], ref["zkey"])
+    np.testing.assert_array_equal(got["bbox"], ref["bbox"])
+
+
+# ------------------------------------------------------------------------------------------------
+# K2: bit-exact bins
+# ------------------------------------------------------------------------------------------------
+def _gpu_bins(B, w, shift, with_members=True, cap=None):
+    sc = _scene(w)
+    from paper_1004_1302_b200.scene import _camera_struct
+    cs, ps = _camera_struct(w.camera), sc.params()
+    bs = 1 << shift
+    T = ((w.camera.width + bs - 1) >> shift) * ((w.camera.height + bs - 1) >> shift)
+    ref = oracle.project_f32(w)
+    order = oracle.depth_order(ref["zkey"], ref["visible"]) if w.mode == ABSORB else None
+    rc, ro, rm = oracle.bins(ref["bbox"], ref["visible"], w.camera.width, w.camera.height, shift, order=order)
+    D = int(ro[-1])
+    cap = D + 7 if cap is None else cap
+    nbytes = B.splotch_debug_workspace_bytes(w.n, cs, ps, shift, cap)
+    ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    cnt = torch.zeros(T, dtype=torch.int32, device="cuda")
+    off = torch.zeros(T + 1, dtype=torch.int64, device="cuda")
+    mem = torch.full((max(cap, 1),), -1, dtype=torch.int32, device="cuda")
+    B.splotch_debug_bins(sc.particles(), w.n, cs, sc.colormap(), ps, sc._aligned(ws), nbytes, shift, cnt, off,
+                         mem if with_members else None, cap if with_members else 0)
+    torch.cuda.synchronize()
+    return (cnt.cpu().numpy().view(np.uint32), off.cpu().numpy().view(np.uint64), mem.cpu().numpy().view(np.uint32)), (rc, ro, rm)
+
+
+@pytest.mark.parametrize("case,shift", [("C1", 4), ("C1", 6), ("C2", 4), ("C2", 6), ("C3", 6)])
+def test_bins_additive_bit_exact(B, case, shift):
+    w = {"C1": lambda: workloads.make("C1"),
+         "C2": lambda: workloads.make("C2", 60_000, width=500, height=333),
+         "C3": lambda: workloads.make("C3", 120_000, width=1024, height=1024)}[case]()
+    (cnt, off, mem), (rc, ro, rm) = _gpu_bins(B, w, shift)
+    np.testing.assert_array_equal(cnt, rc)
+    np.testing.assert_array_equal(off, ro)
+    D = int(ro[-1])
+    assert D > w.n // 2
+    for t in range(len(rc)):                                   # member SET of every bin
+        a, b = int(ro[t]), int(ro[t + 1])
+        np.testing.assert_array_equal(np.sort(mem[a:b]), np.sort(rm[a:b]))
+
+
+@pytest.mark.parametrize("shift", [4, 6])
+def test_bins_absorb_sequence_bit_exact(B, shift):
+    w = workloads.make("C4", 150_000, width=640, height=400)
+    (cnt, off, mem), (rc, ro, rm) = _gpu_bins(B, w, shift)
+    np.testing.assert_array_equal(cnt, rc)
+    np.testing.assert_array_equal(off, ro)
+    D = int(ro[-1])
+    assert D > 10_000
+    np.testing.assert_array_equal(mem[:D], rm)                 # member SEQUENCE: depth order, ties by index
+
+
+def test_bins_member_capacity_is_respected(B):
+    w = workloads.make("C1", 20_000)
+    (cnt, off, mem), (rc, ro, rm) = _gpu_bins(B, w, 4, cap=100)
+    np.testing.assert_array_equal(cnt, rc)
+    np.testing.assert_array_equal(off, ro)
+    assert np.all(mem == np.uint32(0xFFFFFFFF))                # untouched
+
+
+# ------------------------------------------------------------------------------------------------
+# whole path: pixels
+# ------------------------------------------------------------------------------------------------
+def _render_both(w, raw=False, mode=None):
+    sc = _scene(w)
+    out = sc.render(raw=raw, mode=mode)
+    torch.cuda.synchronize()
+    ref = oracle.render(w, raw=raw, mode=mode)
+    return out.cpu().numpy(), ref
+
+
+@pytest.mark.parametrize("raw", [True, False])
+def test_additive_c1_full(B, raw):
+    w = workloads.make("C1")
+    out, ref = _render_both(w, raw=raw)
+    assert ref.max() > 1.0
+    _tol_check(out, ref, "C1")
+
+
+@pytest.mark.parametrize("case", ["C2", "C3", "C5"])
+def test_additive_scaled_configs(B, case):
+    w = {"C2": lambda: workloads.make("C2", 200_000, width=512, height=512),
+         "C3": lambda: workloads.make("C3", 300_000, width=600, height=360),        # ragged: not multiples of 64
+         "C5": lambda: workloads.make("C5", 400_000, width=513, height=257)}[case]()  # odd width: scalar write path
+    out, ref = _render_both(w, raw=True)
+    assert ref.mean() > 0.05
+    _tol_check(out, ref, case)
+    out, ref = _render_both(w, raw=False)
+    _tol_check(out, ref, case)
+
+
+def test_absorb_scaled_c4(B):
+    w = workloads.make("C4", 200_000, width=512, height=384)
+    out, ref = _render_both(w)
+    assert ref.max() > 0.3
+    _tol_check(out, ref, "C4")
+
+
+def test_absorb_with_a_equal_e_matches_additive_oracle(B):
+    w = workloads.make("C1", 50_000, width=200, height=200)
+    w.lut_a = w.lut_e.copy()
+    w.abs_brightness = list(w.brightness)
+    w.mode = ABSORB
+    sc = _scene(w)
+    out = sc.render().cpu().numpy()
+    ref = oracle.render(w, mode=ADDITIVE)
+    _tol_check(out, ref, "absorb(A=E) vs additive")
+
+
+def test_absorb_strong_absorption_and_zero_channel(B):
+    """u = A tau well above 0.25 (exact phi branch) and A_c = 0 in one channel (R15)."""
+    rs = np.random.RandomState(5)
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=96, h=96)
+    n = 400
+    pts = np.stack([rs.uniform(-1.2, 1.2, n), rs.uniform(-1.2, 1.2, n), rs.uniform(-2, 2, n),
+                    rs.uniform(0.05, 0.5, n), rs.uniform(0.5, 3.0, n), rs.uniform(0, 1, n)], 1)
+    lut_e = np.array([[0.2, 0.5, 0.9], [1.0, 0.3, 0.1]], np.float32)
+    lut_a = np.array([[3.0, 0.0, 0.6], [0.5, 0.0, 8.0]], np.float32)
+    w = mk(pts, c, lut_e=lut_e, lut_a=lut_a, mode=ABSORB, support_f=3.2)
+    out, ref = _render_both(w)
+    assert ref.max() > 0.5
+    # pixels whose coverage decision sits on the rim may flip between fp32 and fp64 (DESIGN.md error budget)
+    _tol_check_masked(w, out, ref)
+
+
+def _tol_check_masked(w, out, ref):
+    tab, ok = oracle.splat_table(w)
+    H, W = ref.shape[:2]
+    jj, ii = np.meshgrid(np.arange(H) + 0.5, np.arange(W) + 0.5, indexing="ij")
+    rim = np.zeros((H, W), bool)
+    for p in np.nonzero(ok)[0]:
+        d2 = (ii - tab[p, 0]) ** 2 + (jj - tab[p, 1]) ** 2
+        rim |= np.abs(d2 - tab[p, 3] ** 2) < 1e-4 * tab[p, 3] ** 2
+    err = np.abs(out - ref) / (1e-4 * np.maximum(1.0, np.abs(ref)))
+    assert rim.mean() < 0.05
+    assert err[~rim].max() <= 1.0, err[~rim].max()
+
+
+def test_single_splat_shapes(B):
+    """One bright splat at several sizes (sub-pixel to screen filling), a_c of order one."""
+    for r, f in [(0.0004, 3.1), (0.004, 3.1), (0.04, 3.1), (0.4, 3.1), (4.0, 3.1), (0.02, 5.0)]:
+        c = cam(eye=(0.013, -0.007, -10.0), lookat=(0.013, -0.007, 0.0), fov=20.0, w=200, h=136)
+        w = mk([(0.05, 0.02, 0.0, r, 1.0 / r, 0.3)], c, lut_e=const_lut((1.0, 0.6, 0.3)), support_f=f)
+        out, ref = _render_both(w, raw=True)
+        _tol_check_masked(w, out, ref)
+        assert (ref.max() > 0.5) or r < 0.001
+
+
+def test_edge_cases(B):
+    c = workloads.make("C1", 10).camera
+    # empty input
+    w0 = mk(np.zeros((0, 6)), c)
+    sc = _scene(w0)
+    assert float(sc.render(raw=True).abs().max()) == 0.0
+    # everything culled
+    w1 = mk([(0.5, 0.5, -5.0, 0.01, 1, 0), (np.nan, 0, 0, 0.01, 1, 0)], c)
+    assert float(_scene(w1).render(raw=False).abs().max()) == 0.0
+    # absorb, empty and culled
+    w2 = mk([(0.5, 0.5, -5.0, 0.01, 1, 0)], c, lut_a=const_lut(), mode=ABSORB)
+    assert float(_scene(w2).render().abs().max()) == 0.0
+    # pair capacity too small: error status, zero image, never a partial image
+    w3 = workloads.make("C1", 20_000)
+    sc = _scene(w3)
+    pairs, vis = sc.count_pairs()
+    assert pairs > vis > 10_000
+    sc.reserve(max_pairs=pairs // 2)
+    img = sc.render(check=False)
+    status, v2, p2 = B.splotch_workspace_status(sc._aligned(sc.workspace))
+    assert status == B.SPLOTCH_ERR_WORKSPACE and p2 == pairs and v2 == vis
+    assert float(img.abs().max()) == 0.0
+    with pytest.raises(B.SplotchError):
+        sc.render()
+    # exact capacity works
+    sc.reserve(max_pairs=pairs)
+    assert float(sc.render().abs().max()) > 0.0
+
+
+def test_repeat_calls_and_orbit_cameras(B):
+    """C5's use case: several cameras over one resident particle set; same camera twice gives the same image."""
+    w = workloads.make("C5", 300_000, width=256, height=256)
+    sc = _scene(w)
+    worst_pairs = max(sc.count_pairs(cm)[0] for cm in w.cameras)
+    sc.reserve(max_pairs=worst_pairs)
+    first = None
+    for j, cm in enumerate(w.cameras[:3]):
+        out = sc.render(cam=cm, raw=True).cpu().numpy()
+        ref = oracle.render(w, camera=cm, raw=True)
+        _tol_check(out, ref, f"C5 camera {j}")
+        if j == 0:
+            first = out
+    again = sc.render(cam=w.cameras[0], raw=True).cpu().numpy()
+    np.testing.assert_allclose(again, first, rtol=2e-6, atol=1e-7)   # atomics: order of partial sums may differ
+
+
+def test_stats_counts(B):
+    w = workloads.make("C1")
+    sc = _scene(w)
+    vis, pairs, upd = sc.stats(bin_shift=4)
+    ref = oracle.project_f32(w)
+    _, ro, _ = oracle.bins(ref["bbox"], ref["visible"], 256, 256, 4, with_members=False)
+    assert vis == int(ref["visible"].sum()) and pairs == int(ro[-1])
+    tab, ok = oracle.splat_table(w)
+    # U: covered pixel centres, counted independently in double for a sample of particles
+    idx = np.nonzero(ref["visible"])[0][::50]
+    ws = mk(np.stack([w.x[idx], w.y[idx], w.z[idx], w.r[idx], w.I[idx], w.colval[idx]], 1), w.camera, lut_e=w.lut_e,
+            brightness=w.brightness)
+    _, _, upd_s = _scene(ws).stats(bin_shift=4)
+    jj, ii = np.meshgrid(np.arange(256) + 0.5, np.arange(256) + 0.5, indexing="ij")
+    expect = sum(int(((ii - tab[p, 0]) ** 2 + (jj - tab[p, 1]) ** 2 <= tab[p, 3] ** 2).sum()) for p in idx)
+    assert abs(upd_s - expect) <= max(3, expect // 20000)
+    assert upd > 50 * upd_s * 0.5
+
+
+def test_render_host_matches_device_render(B):
+    w = workloads.make("C3", 200_000, width=320, height=320)
+    sc = _scene(w)
+    dev = sc.render().cpu().numpy()
+    hb = sc.host_buffers()
+    out_host, _ = sc.render_host(hb)
+    np.testing.assert_allclose(out_host.numpy(), dev, rtol=2e-6, atol=1e-7)
+    ref = oracle.render(w)
+    _tol_check(out_host.numpy(), ref, "render_host")

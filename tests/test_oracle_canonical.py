@@ -52,7 +52,7 @@ def test_projector_matches_numpy_float32_sequence():
         i1 = max(min(np.floor((sx + R) - f32(0.5)), c.width - 1), -1)
         j0 = min(max(np.ceil((sy - R) - f32(0.5)), 0), c.height)
         j1 = max(min(np.floor((sy + R) - f32(0.5)), c.height - 1), -1)
-        vis = bool(i0 <= i1 and j0 <= j1 and ss > 0)
+        vis = bool(i0 <= i1 and j0 <= j1 and ss > 0 and np.isfinite(R))
         assert bool(pr["visible"][p]) == vis
         if vis:
             nvis += 1
