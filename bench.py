@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- the Splotch render hot path on B200: Mparticles/s and roofline fractions.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (transform/cull/colour -> bin -> rasterise -> output
+map) over the resident synthetic particle set of the workload.  The default workload is C3, the
+100M-particle additive config BASELINE.json's north_star quotes its target on.  One JSON line is
+printed on stdout (rank 0); everything else goes to stderr.
+
+N > 1 (torchrun, one rank per GPU): additive mode shards by particles exactly like the paper's
+MPI layer: every rank renders its own particle set into a raw-S partial image,
+one NCCL all-reduce sums the partial images, then the output map is applied.  Weak scaling:
+every rank holds a full-size particle set generated from its own seed.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "Mparticles/s rendered and achieved HBM GB/s fraction on one B200"
+SM_COUNT_NOMINAL = 148
+LANES_PER_SM = 128
+ALGO_LANE_OPS_PER_UPDATE = {0: 5.0, 1: 17.0}   # 1 mul + 3 FMA + 1 test; absorb adds 3 exp + ~9 ops
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+        except Exception:  # pragma: no cover
+            pass
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def make_workload(name: str, n, rank: int):
+    import workloads
+    kw = {}
+    if rank > 0:
+        kw["seed"] = {"C1": 1004130201, "C2": 1004130202, "C3": 1004130203, "C4": 1004130202, "C5": 1004130205}[name] + 1000 * rank
+    t = time.time()
+    w = workloads.make(name, n, **kw)
+    log(f"[bench] rank {rank}: generated {name} n={w.n} in {time.time() - t:.1f}s")
+    return w
+
+
+def oracle_sample(w, target_seconds: float):
+    """Bounded sample of the workload for the CPU oracle: a strided subsample at full resolution,
+    stride chosen from a short calibration run so that one render takes about target_seconds."""
+    import oracle
+    cores = oracle.max_threads()
+    probe = w.subsample(4096)
+    t = time.time()
+    oracle.render(probe)
+    dt = max(time.time() - t, 1e-3)
+    per_particle = dt / probe.n
+    stride = int(np.ceil(per_particle * w.n / target_seconds))
+    stride = max(1, min(stride, 4096))
+    return w.subsample(stride), stride, cores
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (as it stands) on a bounded sample of the same workload."""
+    import oracle
+    w = make_workload(args.workload, args.n, 0)
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    ws, stride, cores = oracle_sample(w, min(25.0, budget))
+    for _ in range(args.warmup):
+        oracle.render(ws)
+    t = time.time()
+    for _ in range(args.steps):
+        oracle.render(ws)
+    dt = (time.time() - t) / max(1, args.steps)
+    val = ws.n / dt / 1e6
+    cam = w.camera
+    line = dict(impl="reference", metric=METRIC, value=val, unit="Mparticles/s", n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic",
+                config=dict(workload=f"{w.name}: {w.n} particles, {cam.width}x{cam.height}, "
+                                     f"{'absorb' if w.mode else 'additive'} mode", sample=f"1-in-{stride} strided subsample"),
+                cpu_baseline=dict(value=val, unit="Mparticles/s", cores=cores, kind="oracle",
+                                  sample=f"1-in-{stride} particle-strided subsample ({ws.n} particles) at full resolution"),
+                e2e=dict(value=val, unit="Mparticles/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--n", type=int, default=None, help="particle count (default: the config's full size)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    from paper_1004_1302_b200 import Scene, binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    peaks = read_peaks()
+    w = make_workload(args.workload, args.n, rank)
+    if world > 1 and w.mode != 0:
+        raise SystemExit("multi-GPU sharding is defined for the additive mode only (DESIGN.md 'Multi-GPU')")
+    cam = w.camera
+    sc = Scene(w, dev)
+    vis, pairs, updates = sc.stats()
+    sc.reserve(max_pairs=pairs + 1024)
+    log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g}, "
+        f"workspace {sc.workspace.numel() / 2**30:.2f} GiB")
+    out = torch.empty((cam.height, cam.width, 3), dtype=torch.float32, device=dev)
+    raw = world > 1
+
+    def step():
+        sc.render(cam, raw=raw, out=out, check=False)
+        if world > 1:                              # one collective reduction of the partial images
+            dist.all_reduce(out)
+            B.splotch_normalize(out, out, out.numel())
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    status, _, _ = B.splotch_workspace_status(sc._aligned(sc.workspace))
+    assert status == B.SPLOTCH_OK, "workspace too small"
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    launches0 = B.splotch_launch_count()
+    B.splotch_profile_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    stage_ms, prof_calls = B.splotch_profile_read()
+    B.splotch_profile_enable(False)
+    launches = B.splotch_launch_count() - launches0
+    clocks = sampler.stop()
+    ms_step = ms_total / max(1, args.steps)
+    if world > 1:
+        t = torch.tensor([ms_step], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+        tl = torch.tensor([launches], dtype=torch.int64, device=dev)
+        dist.all_reduce(tl)
+        launches = int(tl.item())
+    total_particles = w.n * world
+    value = total_particles / (ms_step * 1e-3) / 1e6
+
+    # ---- roofline of the dominant kernel (K3, the tile rasteriser): plain FP32 ALU bound ----
+    raster_ms = stage_ms[3]
+    sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    alu_peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12          # Tlane-op/s
+    c_ops = ALGO_LANE_OPS_PER_UPDATE[w.mode]
+    alu_achieved = updates * c_ops / (raster_ms * 1e-3) / 1e12 if raster_ms > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(w.name)
+        except Exception:
+            traffic = None
+    roofline = dict(bound="alu", kernel="raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel",
+                    achieved=alu_achieved, peak=alu_peak, unit="Tlane-op/s", frac=alu_achieved / alu_peak if alu_peak else None,
+                    traffic=traffic, kernel_ms=raster_ms, kernel_share_of_step=raster_ms / ms_step if ms_step else None,
+                    updates_per_launch=updates, algorithmic_lane_ops_per_update=c_ops,
+                    peak_source=f"{sm_count} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} clock)")
+    algo_bytes = w.n * w.bytes_per_particle + cam.width * cam.height * 12
+    hbm_gbs = algo_bytes / (ms_step * 1e-3) / 1e9
+    hbm = dict(algorithmic_bytes_per_step=algo_bytes, achieved_gbs=hbm_gbs, frac_of_measured=hbm_gbs / peaks["hbm_gbs"],
+               frac_of_nominal_8TBs=hbm_gbs / 8000.0, peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"])
+
+    # ---- end to end through the C ABI with host buffers (H2D + render + D2H inside the call) ----
+    e2e = None
+    if not args.no_e2e and world == 1:
+        hb = sc.host_buffers()
+        out_host = torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory()
+        sc.workspace = None
+        torch.cuda.empty_cache()
+        _, hws = sc.render_host(hb, cam, out_host=out_host, max_pairs=pairs + 1024)
+        n_e2e = max(1, min(args.steps, 3))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            sc.render_host(hb, cam, out_host=out_host, max_pairs=pairs + 1024, workspace=hws)
+        dt = (time.perf_counter() - t0) / n_e2e
+        e2e = dict(value=w.n / dt / 1e6, unit="Mparticles/s", h2d_bytes_per_step=sc.h2d_bytes(),
+                   d2h_bytes_per_step=cam.width * cam.height * 12, ms_per_step=dt * 1e3, steps=n_e2e,
+                   call="splotch_render_host (pinned host buffers; copies inside the timed call)")
+        del hws
+    elif world > 1:
+        e2e = dict(value=None, unit="Mparticles/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0,
+                   note="end-to-end host-buffer path is measured at N=1")
+
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only ----
+    cpu = None
+    if not args.no_cpu_baseline and world == 1 and rank == 0:
+        import oracle
+        ws_, stride, cores = oracle_sample(w, 15.0)
+        t0 = time.time()
+        oracle.render(ws_)
+        dt = time.time() - t0
+        cpu = dict(value=ws_.n / dt / 1e6, unit="Mparticles/s", cores=cores, kind="oracle", seconds=dt,
+                   sample=f"1-in-{stride} particle-strided subsample ({ws_.n} particles) of {w.name} at full resolution "
+                          f"(subsample measurement)")
+
+    if rank == 0:
+        line = dict(metric=METRIC, value=value, unit="Mparticles/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                    data="synthetic",
+                    config=dict(workload=f"{w.name}: {w.n} particles/GPU, {cam.width}x{cam.height}, "
+                                         f"{'absorb' if w.mode else 'additive'} mode, f={w.support_f}",
+                                parallelism=f"particle shards x{world} + all-reduce of raw S" if world > 1 else "single GPU",
+                                l2="inputs (particle arrays + splat records + pair list) exceed the 126 MB L2 many times over; no flush needed",
+                                seed=w.seed, visible=vis, pairs=pairs, pixel_updates=updates,
+                                pixels_per_s=cam.width * cam.height / (ms_step * 1e-3),
+                                updates_per_s=updates * world / (ms_step * 1e-3)),
+                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, hbm_roofline=hbm,
+                    stage_ms=dict(zip(["project_count", "offsets", "lists", "raster", "output_map"], stage_ms)),
+                    cpu_baseline=cpu)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

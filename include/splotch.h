@@ -205,6 +205,18 @@ uint64_t splotch_sort_scratch_bytes(int64_t n);
 int splotch_debug_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
                              int32_t key_bits, void *scratch, uint64_t scratch_bytes, void *stream);
 
+/* Per-stage timing of splotch_render with CUDA events recorded on the caller's stream (used by
+ * bench.py for the roofline of the dominant kernel).  splotch_profile_enable(1) resets the
+ * record; while enabled every splotch_render records 6 events (up to 256 calls).
+ * splotch_profile_read SYNCHRONISES on the last recorded event and returns the mean
+ * milliseconds per call of the 5 stages: [0] transform/cull/colour + bin count (K1),
+ * [1] offsets scan + work units, [2] lists (scatter, or depth sort + ordered split),
+ * [3] tile rasteriser (K3), [4] output map / merge (K4).
+ * splotch_launch_count: kernels launched by this library in this process so far. */
+int splotch_profile_enable(int on);
+int splotch_profile_read(double *stage_ms /* host, 5 doubles */, int64_t *calls /* host */);
+unsigned long long splotch_launch_count(void);
+
 const char *splotch_status_string(int status);
 int splotch_last_cuda_error(void);  /* cudaError_t of the last failing CUDA call in this thread */
 int splotch_version(void);

@@ -32,7 +32,8 @@ EXPORTS = [
     "splotch_normalize", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
     "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_scan",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
-    "splotch_last_cuda_error", "splotch_version",
+    "splotch_last_cuda_error", "splotch_version", "splotch_profile_enable", "splotch_profile_read",
+    "splotch_launch_count",
 ]
 
 
@@ -78,6 +79,7 @@ def _lib():
         lib.splotch_status_string.restype = C.c_char_p
         lib.splotch_sort_scratch_bytes.restype = C.c_uint64
         lib.splotch_sort_scratch_bytes.argtypes = [C.c_int64]
+        lib.splotch_launch_count.restype = C.c_ulonglong
         _LIB = lib
     return _LIB
 
@@ -268,3 +270,19 @@ def splotch_debug_sort_pairs(keys, vals, keys_tmp, vals_tmp, n: int, key_bits: i
            _lib().splotch_debug_sort_pairs(_vp(_ptr(keys)), _vp(_ptr(vals)), _vp(_ptr(keys_tmp)), _vp(_ptr(vals_tmp)),
                                            C.c_int64(n), C.c_int32(key_bits), _vp(_ptr(scratch)),
                                            C.c_uint64(scratch_bytes), _vp(_stream(stream))))
+
+
+def splotch_profile_enable(on: bool) -> None:
+    _check("splotch_profile_enable", _lib().splotch_profile_enable(C.c_int(1 if on else 0)))
+
+
+def splotch_profile_read():
+    """(list of 5 mean stage times in ms, number of profiled calls); synchronises."""
+    ms = (C.c_double * 5)()
+    calls = C.c_int64(0)
+    _check("splotch_profile_read", _lib().splotch_profile_read(ms, C.byref(calls)))
+    return [float(v) for v in ms], int(calls.value)
+
+
+def splotch_launch_count() -> int:
+    return int(_lib().splotch_launch_count())

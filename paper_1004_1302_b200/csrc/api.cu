@@ -10,6 +10,34 @@
 namespace splotch {
 
 thread_local int g_last_cuda_error = 0;
+unsigned long long g_launch_count = 0;
+
+// ---------------------------------------------------------------------------------------------
+// optional per-stage timing of splotch_render with CUDA events on the caller's stream
+// ---------------------------------------------------------------------------------------------
+namespace {
+constexpr int kStages = 5;          // project+count | offsets | lists | raster | output map
+constexpr int kMaxProfiledCalls = 256;
+struct Profile {
+    bool on = false;
+    int calls = 0;
+    cudaEvent_t ev[kMaxProfiledCalls][kStages + 1];
+    bool created[kMaxProfiledCalls] = {};
+} g_prof;
+
+void prof_mark(int stage, cudaStream_t st)
+{
+    if (!g_prof.on || g_prof.calls >= kMaxProfiledCalls) return;
+    const int c = g_prof.calls;
+    if (!g_prof.created[c]) {
+        for (int k = 0; k <= kStages; ++k)
+            if (cudaEventCreate(&g_prof.ev[c][k]) != cudaSuccess) { g_prof.on = false; return; }
+        g_prof.created[c] = true;
+    }
+    cudaEventRecord(g_prof.ev[c][stage], st);
+    if (stage == kStages) ++g_prof.calls;
+}
+}  // namespace
 
 int sm_count()
 {
@@ -196,7 +224,7 @@ int setup(const splotch_particles *particles, int64_t n, const splotch_camera *c
 
 // K1 + bin counts + offsets + units: everything up to (not including) the list
 int run_front(const Ctx &c, const splotch_particles *particles, int64_t n, const splotch_colormap *cm,
-              uint64_t max_pairs, uint32_t chunk, const DebugProjectOut *dbg)
+              uint64_t max_pairs, uint32_t chunk, const DebugProjectOut *dbg, bool profiled = false)
 {
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.head, 0, 256, c.st));
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_count, 0, (size_t)c.n_bins * 4, c.st));
@@ -207,6 +235,7 @@ int run_front(const Ctx &c, const splotch_particles *particles, int64_t n, const
                             c.at<uint32_t>(c.L.bin_count), c.rc.mode == SPLOTCH_ABSORB ? c.at<uint32_t>(c.L.zkeys) : nullptr,
                             c.head(), dbg, c.st);
     if (rc) return rc;
+    if (profiled) prof_mark(1, c.st);
     rc = launch_scan_u32_u64(c.at<uint32_t>(c.L.bin_count), c.at<uint64_t>(c.L.bin_offset), c.n_bins,
                              c.ws + c.L.scan_scratch, c.st);
     if (rc) return rc;
@@ -327,16 +356,20 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
     if (rc) return rc;
     const bool absorb = c.rc.mode == SPLOTCH_ABSORB;
     const int64_t n_values = (int64_t)c.cam.W * c.cam.H * 3;
-    rc = run_front(c, particles, n, colormap, max_pairs, absorb ? kChunkAbs : kChunkAdd, nullptr);
+    prof_mark(0, c.st);
+    rc = run_front(c, particles, n, colormap, max_pairs, absorb ? kChunkAbs : kChunkAdd, nullptr, true);
     if (rc) return rc;
+    prof_mark(2, c.st);
     uint32_t *list = nullptr;
     rc = run_lists(c, n, max_pairs, &list);
     if (rc) return rc;
+    if (!absorb) SPLOTCH_CUDA_TRY(cudaMemsetAsync(out_rgb, 0, (size_t)n_values * 4, c.st));
+    prof_mark(3, c.st);
     if (!absorb) {
-        SPLOTCH_CUDA_TRY(cudaMemsetAsync(out_rgb, 0, (size_t)n_values * 4, c.st));
         rc = launch_raster_additive(c.at<SplatAdd>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
                                     c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
         if (rc) return rc;
+        prof_mark(4, c.st);
         if (!(params->flags & SPLOTCH_RAW_SUM)) {
             rc = launch_normalize(out_rgb, out_rgb, n_values, c.st);
             if (rc) return rc;
@@ -345,13 +378,41 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
         rc = launch_raster_absorb(c.at<SplatAbs>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
                                   c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, c.at<float>(c.L.partials), c.head(), c.st);
         if (rc) return rc;
+        prof_mark(4, c.st);
         rc = launch_merge_absorb(c.at<float>(c.L.partials), c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
         if (rc) return rc;
     }
     zero_if_failed_kernel<<<sm_count() * 4, 256, 0, c.st>>>(out_rgb, (long long)n_values, c.head());
     SPLOTCH_LAUNCH_CHECK();
+    prof_mark(kStages, c.st);
     return SPLOTCH_OK;
 }
+
+int splotch_profile_enable(int on)
+{
+    g_prof.on = on != 0;
+    g_prof.calls = 0;
+    return SPLOTCH_OK;
+}
+
+int splotch_profile_read(double *stage_ms, int64_t *calls)
+{
+    if (!stage_ms) return SPLOTCH_ERR_INVALID_ARG;
+    for (int k = 0; k < kStages; ++k) stage_ms[k] = 0.0;
+    const int n = g_prof.calls;
+    if (calls) *calls = n;
+    if (n == 0) return SPLOTCH_OK;
+    SPLOTCH_CUDA_TRY(cudaEventSynchronize(g_prof.ev[n - 1][kStages]));
+    for (int c = 0; c < n; ++c)
+        for (int k = 0; k < kStages; ++k) {
+            float ms = 0.f;
+            SPLOTCH_CUDA_TRY(cudaEventElapsedTime(&ms, g_prof.ev[c][k], g_prof.ev[c][k + 1]));
+            stage_ms[k] += (double)ms / n;
+        }
+    return SPLOTCH_OK;
+}
+
+unsigned long long splotch_launch_count(void) { return g_launch_count; }
 
 int splotch_workspace_status(const void *workspace, void *stream, int32_t *status, uint64_t *visible, uint64_t *pairs)
 {

@@ -97,7 +97,12 @@ extern thread_local int g_last_cuda_error;
         }                                                        \
     } while (0)
 
-#define SPLOTCH_LAUNCH_CHECK() SPLOTCH_CUDA_TRY(cudaGetLastError())
+extern unsigned long long g_launch_count;   // kernels this library has launched (bench.py "gpu_launches")
+#define SPLOTCH_LAUNCH_CHECK()                      \
+    do {                                            \
+        ++::splotch::g_launch_count;                \
+        SPLOTCH_CUDA_TRY(cudaGetLastError());       \
+    } while (0)
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 int sm_count();

@@ -208,7 +208,7 @@ def _render_both(w, raw=False, mode=None):
 def test_additive_c1_full(B, raw):
     w = workloads.make("C1")
     out, ref = _render_both(w, raw=raw)
-    assert ref.max() > 1.0
+    assert ref.max() > (1.0 if raw else 0.9)
     _tol_check(out, ref, "C1")
 
 
@@ -278,7 +278,7 @@ def test_single_splat_shapes(B):
         w = mk([(0.05, 0.02, 0.0, r, 1.0 / r, 0.3)], c, lut_e=const_lut((1.0, 0.6, 0.3)), support_f=f)
         out, ref = _render_both(w, raw=True)
         _tol_check_masked(w, out, ref)
-        assert (ref.max() > 0.5) or r < 0.001
+        assert ref.max() > 0.05 or r < 0.001
 
 
 def test_edge_cases(B):
