@@ -1,0 +1,67 @@
+// raster_common.cuh -- helpers shared by the two tile rasterisers (additive, absorb).
+#pragma once
+#include "common.cuh"
+
+namespace splotch {
+
+namespace {
+
+constexpr int kBatch = 32;
+constexpr float kLog2e = 1.4426950408889634f;
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ void red_add_v4(float *addr, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d)
+                 : "memory");
+}
+
+// class of a tw x th tile of pixel centres against the truncation circle: 0 outside, 1 rim, 2 inside.
+// The margins make the classification conservative: a tile is only called inside/outside when
+// every pixel of it is, whatever the rounding of the per-pixel test.
+__device__ __forceinline__ int classify_tile(float sx, float sy, float R, float x_lo, float y_lo, int W, int H,
+                                             int px0, int py0, float tw = 16.0f, float th = 16.0f)
+{
+    if (px0 >= W || py0 >= H) return 0;
+    const float x_hi = x_lo + (tw - 1.0f), y_hi = y_lo + (th - 1.0f);
+    const float nx = fmaxf(fmaxf(x_lo - sx, sx - x_hi), 0.0f), ny = fmaxf(fmaxf(y_lo - sy, sy - y_hi), 0.0f);
+    const float fx = fmaxf(sx - x_lo, x_hi - sx), fy = fmaxf(sy - y_lo, y_hi - sy);
+    const float R2 = R * R;
+    if (nx * nx + ny * ny > R2 * 1.00001f) return 0;
+    if (fx * fx + fy * fy < R2 * 0.99999f) return 2;
+    return 1;
+}
+
+struct UnitInfo {
+    int bin;
+    uint32_t count;
+    unsigned long long first;
+};
+
+// largest b with unit_prefix[b] <= unit (bins without units share their prefix with the next one)
+__device__ __forceinline__ int find_bin(const uint32_t *__restrict__ unit_prefix, int n_bins, uint32_t unit)
+{
+    int lo = 0, hi = n_bins;            // invariant: prefix[lo] <= unit < prefix[hi]
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(unit_prefix + mid) <= unit) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+}  // namespace
+}  // namespace splotch
