@@ -1,15 +1,20 @@
 // raster_add.cu -- K3 tile rasteriser of the additive mode + K4 output map (steps a8, a9).
 //
 // One CTA (8 warps) owns a 64x64-pixel block of the screen for the duration of a work unit (a
-// chunk of that block's splat list).  Each warp owns a 32x16 tile, each lane 8 consecutive
-// pixels in each of 2 rows: 48 accumulators in REGISTERS.  Per batch of 32 splats the CTA
+// chunk of that block's splat list).  The block is cut into sixteen 16x16 tiles; every warp owns
+// TWO of them, far apart ((tx + 2 ty) mod 8 == warp), so that the compact cluster of tiles a splat
+// touches spreads over many warps.  A lane owns 8 consecutive pixels of one tile row in each of
+// its two tiles: 48 accumulators in REGISTERS, held as 24 packed f32x2 pairs.
+// Per batch of 32 splats the CTA
 //   (i)   gathers the 32-byte splat records into shared memory with cp.async, double buffered;
 //   (ii)  evaluates the separable Gaussian once per splat: exp(-d^2/s^2) = gx[i] * gy[j]; it
 //         stores gx[64] and, per row j, the record (a_r gy[j], a_g gy[j], a_b gy[j], thr / gy[j]),
 //         and classifies every (splat, tile) pair as outside / rim / inside the truncation circle;
-//   (iii) lets every warp walk only the splats that touch its tile.  Inside tiles cost 3 FMA per
-//         pixel update (acc_c += (a_c gy[j]) * gx[i]); rim tiles add one compare per pixel
-//         (d^2 <= R^2  <=>  gx[i] >= thr / gy[j],  thr = exp(-f^2)) and predicate the FMAs.
+//   (iii) lets every warp walk only the (splat, tile) pairs that touch its tiles.  A pair costs
+//         three 128-bit shared loads and 12 FFMA2 (acc_c += (gx[i], gx[i+1]) * (a_c gy[j])): 3 FMA
+//         per pixel update in half the issue slots.  Rim tiles first zero the gx of uncovered
+//         pixels (d^2 <= R^2  <=>  gx[i] >= thr / gy[j],  thr = exp(-f^2)): two ALU-pipe
+//         instructions per pixel that overlap the FMA pipe of the other warps.
 // The block is added to the raw image once per unit with vector red.global.add: any summation
 // order is legal when A = E.
 #include "raster_common.cuh"
@@ -19,35 +24,44 @@ namespace splotch {
 namespace {
 
 constexpr int kRasThreads = 256;
-constexpr int kWarps = kRasThreads / 32;
-constexpr int kTileW = 32, kTileH = 16;         // warp tile; lane = 8 columns x 2 rows (rows r and r + 8)
-
-// packed fp32x2 arithmetic (sm_100+): one FFMA2 issues two FMAs, halving the issue slots of the
-// inner loop; the FMA pipe rate is unchanged (measured: 36 Tlane-FMA/s either way)
-__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
-{
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(unsigned long long v, float &lo, float &hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ void fma2_acc(unsigned long long &c, unsigned long long a, unsigned long long b)
-{
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));      // c += a * b, in place
-}
+constexpr int kTiles = 16;                      // 16x16-pixel tiles of a block, index ty * 4 + tx
+constexpr uint32_t kTileA = 0xBA763210u;        // nibble w: first tile of warp w  ((tx + 2 ty) mod 8 == w)
+constexpr uint32_t kTileB = 0xDC9854FEu;        // nibble w: second tile of warp w
 
 struct SmemAdd {
     float4 row[2][kBatch][kBlockPx];            // (a_r gy, a_g gy, a_b gy, thr / gy) per splat and block row
     float gx[2][kBatch][kBlockPx];              // per splat and block column
     SplatAdd rec[2][kBatch];
     uint32_t ids[kChunkAdd];
-    unsigned char cls[2][kBatch][kWarps];
+    unsigned char cls[2][kBatch][kTiles];
     UnitInfo unit;
     uint32_t unit_id;
 };
+
+// one (splat, tile) pair: this lane's 8 pixels of row `y` of the tile, channels packed as f32x2
+template <bool kRim>
+__device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const float4 *__restrict__ rows, int x, int y,
+                                           float2 (&acc)[3][4])
+{
+    const float4 g0 = *reinterpret_cast<const float4 *>(gxs + x);
+    const float4 g1 = *reinterpret_cast<const float4 *>(gxs + x + 4);
+    const float4 r = rows[y];
+    float2 p[4] = { make_float2(g0.x, g0.y), make_float2(g0.z, g0.w), make_float2(g1.x, g1.y), make_float2(g1.z, g1.w) };
+    if (kRim) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            p[q].x = p[q].x >= r.w ? p[q].x : 0.0f;
+            p[q].y = p[q].y >= r.w ? p[q].y : 0.0f;
+        }
+    }
+    const float2 wr = make_float2(r.x, r.x), wg = make_float2(r.y, r.y), wb = make_float2(r.z, r.z);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        acc[0][q] = __ffma2_rn(p[q], wr, acc[0][q]);
+        acc[1][q] = __ffma2_rn(p[q], wg, acc[1][q]);
+        acc[2][q] = __ffma2_rn(p[q], wb, acc[2][q]);
+    }
+}
 
 __global__ void __launch_bounds__(kRasThreads, 2)
 raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
@@ -57,8 +71,10 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SmemAdd &sm = *reinterpret_cast<SmemAdd *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int lx = (warp & 1) * kTileW + (lane & 3) * 8;     // first of this lane's 8 columns inside the block
-    const int ly = (warp >> 1) * kTileH + (lane >> 2);       // this lane's rows inside the block: ly and ly + 8
+    const int tA = (kTileA >> (4 * warp)) & 15, tB = (kTileB >> (4 * warp)) & 15;
+    const int lr = lane & 15, lc = (lane >> 4) * 8;          // row inside a tile, first of 8 columns inside a tile
+    const int xA = (tA & 3) * kTilePx + lc, yA = (tA >> 2) * kTilePx + lr;   // block-relative
+    const int xB = (tB & 3) * kTilePx + lc, yB = (tB >> 2) * kTilePx + lr;
     const uint32_t n_units = head->n_units;
 
     while (true) {
@@ -94,18 +110,18 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
             }
             cp_async_commit();
         };
-        // 8 threads per splat: each 8 gx values, 8 row records and the class of one warp tile
+        // 8 threads per splat: each 8 gx values, 8 row records and the class of two tiles
         auto produce = [&](int b, int slot) {
             const int s = tid >> 3, part = tid & 7;
             const uint32_t e = (uint32_t)b * kBatch + s;
             if (b >= n_batches || e >= count) {
-                sm.cls[slot][s][part] = 0;
+                *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = 0;
                 return;
             }
             const float4 g = *reinterpret_cast<const float4 *>(&sm.rec[slot][s]);        // sx, sy, c, R
             const float4 a = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 1);  // a_r, a_g, a_b, bins
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {           // columns part*4 + 32h .. +3
+            for (int h = 0; h < 2; ++h) {           // columns part*4 + 32h .. +3: conflict-free 128-bit stores
                 const float x0 = (float)(px0 + part * 4 + 32 * h) + 0.5f;
                 float4 v;
                 float t;
@@ -116,15 +132,20 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                 *reinterpret_cast<float4 *>(&sm.gx[slot][s][part * 4 + 32 * h]) = v;
             }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {           // rows part + 8k: conflict-free 128-bit stores
+            for (int k = 0; k < 8; ++k) {           // rows part + 8k
                 const int j = part + 8 * k;
                 const float t = ((float)(py0 + j) + 0.5f - g.y) * g.z;
                 const float gy = ex2_approx(-t * t);
                 sm.row[slot][s][j] = make_float4(a.x * gy, a.y * gy, a.z * gy, __fdividef(thr, gy));
             }
-            const int tpx = px0 + (part & 1) * kTileW, tpy = py0 + (part >> 1) * kTileH;
-            sm.cls[slot][s][part] = (unsigned char)classify_tile(g.x, g.y, g.w, (float)tpx + 0.5f, (float)tpy + 0.5f, W, H,
-                                                                 tpx, tpy, (float)kTileW, (float)kTileH);
+            unsigned short c2 = 0;
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const int t = 2 * part + k;
+                const int tpx = px0 + (t & 3) * kTilePx, tpy = py0 + (t >> 2) * kTilePx;
+                c2 |= (unsigned short)(classify_tile(g.x, g.y, g.w, (float)tpx + 0.5f, (float)tpy + 0.5f, W, H, tpx, tpy) << (8 * k));
+            }
+            *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = c2;
         };
 
         gather(0, 0);
@@ -134,80 +155,40 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
         produce(0, 0);
         __syncthreads();
 
-        // accumulators: acc[h][c][q] = pixels (2q, 2q+1) of row h, channel c, packed as f32x2
-        unsigned long long acc[2][3][4];
+        float2 accA[3][4], accB[3][4];              // [channel][pixel pair]
 #pragma unroll
-        for (int h = 0; h < 2; ++h)
+        for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) acc[h][c][q] = 0ull;
+            for (int q = 0; q < 4; ++q) accA[c][q] = accB[c][q] = make_float2(0.0f, 0.0f);
 
         for (int b = 0; b < n_batches; ++b) {
             const int slot = b & 1;
             gather(b + 2, slot);                 // rec[slot] held batch b, already turned into factors
             produce(b + 1, slot ^ 1);
-            const unsigned char c = sm.cls[slot][lane][warp];
-            unsigned m_in = __ballot_sync(0xffffffffu, c == 2);
-            unsigned m_rim = __ballot_sync(0xffffffffu, c == 1);
-            while (m_in) {                       // tiles entirely inside the circle: no coverage test
-                const int s = __ffs(m_in) - 1;
-                m_in &= m_in - 1;
-                const float4 g0 = *reinterpret_cast<const float4 *>(&sm.gx[slot][s][lx]);
-                const float4 g1 = *reinterpret_cast<const float4 *>(&sm.gx[slot][s][lx + 4]);
-                const float4 r0 = sm.row[slot][s][ly];
-                const float4 r1 = sm.row[slot][s][ly + 8];
-                const unsigned long long gp[4] = { pack2(g0.x, g0.y), pack2(g0.z, g0.w), pack2(g1.x, g1.y), pack2(g1.z, g1.w) };
-                const float w0[3] = { r0.x, r0.y, r0.z }, w1[3] = { r1.x, r1.y, r1.z };
-#pragma unroll
-                for (int ch = 0; ch < 3; ++ch) {
-                    const unsigned long long b0 = pack2(w0[ch], w0[ch]), b1 = pack2(w1[ch], w1[ch]);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {    // two pixels per FFMA2: half the issue slots of scalar FFMA
-                        fma2_acc(acc[0][ch][q], gp[q], b0);
-                        fma2_acc(acc[1][ch][q], gp[q], b1);
-                    }
-                }
-            }
-            while (m_rim) {                      // tiles cut by the circle: d^2 <= R^2 <=> gx >= thr / gy
-                const int s = __ffs(m_rim) - 1;
-                m_rim &= m_rim - 1;
-                const float4 g0 = *reinterpret_cast<const float4 *>(&sm.gx[slot][s][lx]);
-                const float4 g1 = *reinterpret_cast<const float4 *>(&sm.gx[slot][s][lx + 4]);
-                const float4 r0 = sm.row[slot][s][ly];
-                const float4 r1 = sm.row[slot][s][ly + 8];
-                const float gx[8] = { g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w };
-                const float w0[3] = { r0.x, r0.y, r0.z }, w1[3] = { r1.x, r1.y, r1.z };
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    float lo, hi;
-#pragma unroll
-                    for (int ch = 0; ch < 3; ++ch) {
-                        unpack2(acc[0][ch][q], lo, hi);
-                        if (gx[2 * q] >= r0.w) lo = fmaf(w0[ch], gx[2 * q], lo);
-                        if (gx[2 * q + 1] >= r0.w) hi = fmaf(w0[ch], gx[2 * q + 1], hi);
-                        acc[0][ch][q] = pack2(lo, hi);
-                        unpack2(acc[1][ch][q], lo, hi);
-                        if (gx[2 * q] >= r1.w) lo = fmaf(w1[ch], gx[2 * q], lo);
-                        if (gx[2 * q + 1] >= r1.w) hi = fmaf(w1[ch], gx[2 * q + 1], hi);
-                        acc[1][ch][q] = pack2(lo, hi);
-                    }
-                }
-            }
+            const unsigned cA = sm.cls[slot][lane][tA], cB = sm.cls[slot][lane][tB];
+            unsigned m;
+            m = __ballot_sync(0xffffffffu, cA == 2);
+            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
+            m = __ballot_sync(0xffffffffu, cB == 2);
+            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
+            m = __ballot_sync(0xffffffffu, cA == 1);
+            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
+            m = __ballot_sync(0xffffffffu, cB == 1);
+            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
             cp_async_wait_all();
             __syncthreads();
         }
 
-        // write the block once: S += acc (RGB interleaved in the image)
-        const int X0 = px0 + lx;
+        // write the two tiles once: S += acc (RGB interleaved in the image)
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
+            float2 (&acc)[3][4] = h ? accB : accA;
             float v[24];
 #pragma unroll
-            for (int ch = 0; ch < 3; ++ch)
+            for (int c = 0; c < 3; ++c)
 #pragma unroll
-                for (int q = 0; q < 4; ++q) unpack2(acc[h][ch][q], v[3 * (2 * q) + ch], v[3 * (2 * q + 1) + ch]);
-            const int Y = py0 + ly + 8 * h;
+                for (int q = 0; q < 4; ++q) { v[3 * (2 * q) + c] = acc[c][q].x; v[3 * (2 * q + 1) + c] = acc[c][q].y; }
+            const int X0 = px0 + (h ? xB : xA), Y = py0 + (h ? yB : yA);
             if (Y < H && X0 < W) {
                 float *dst = S + ((size_t)Y * W + X0) * 3;
                 if (vec_ok && X0 + 8 <= W) {
