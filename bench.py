@@ -50,6 +50,18 @@ def read_peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def read_traffic(workload: str, kernel: str):
+    """dram read + write bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.csv)."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    for row in csv.DictReader(open(path)):
+        if row["workload"] == workload and row["kernel"] == kernel:
+            return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -241,13 +253,7 @@ def main():
     alu_peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12          # Tlane-op/s
     c_ops = ALGO_LANE_OPS_PER_UPDATE[w.mode]
     alu_achieved = updates * c_ops / (raster_ms * 1e-3) / 1e12 if raster_ms > 0 else 0.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(w.name)
-        except Exception:
-            traffic = None
+    traffic = read_traffic(w.name, "raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel")
     roofline = dict(bound="alu", kernel="raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel",
                     achieved=alu_achieved, peak=alu_peak, unit="Tlane-op/s", frac=alu_achieved / alu_peak if alu_peak else None,
                     traffic=traffic, kernel_ms=raster_ms, kernel_share_of_step=raster_ms / ms_step if ms_step else None,
