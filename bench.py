@@ -166,6 +166,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-tensor", action="store_true", help="additive mode: SPLOTCH_NO_TENSOR (everything on the FP32 ALUs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -195,6 +196,7 @@ def main():
         raise SystemExit("multi-GPU sharding is defined for the additive mode only (DESIGN.md 'Multi-GPU')")
     cam = w.camera
     sc = Scene(w, dev)
+    sc.tensor = not args.no_tensor
     vis, pairs, updates = sc.stats()
     sc.reserve(max_pairs=pairs + 1024)
     log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g}, "
@@ -248,7 +250,7 @@ def main():
     value = total_particles / (ms_step * 1e-3) / 1e6
 
     # ---- roofline of the dominant kernel (K3, the tile rasteriser): plain FP32 ALU bound ----
-    raster_ms = stage_ms[3]
+    raster_ms = stage_ms[3] + stage_ms[4]
     sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
     alu_peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12          # Tlane-op/s
     c_ops = ALGO_LANE_OPS_PER_UPDATE[w.mode]
@@ -310,7 +312,7 @@ def main():
                                 pixels_per_s=cam.width * cam.height / (ms_step * 1e-3),
                                 updates_per_s=updates * world / (ms_step * 1e-3)),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, hbm_roofline=hbm,
-                    stage_ms=dict(zip(["project_count", "offsets", "lists", "raster", "output_map"], stage_ms)),
+                    stage_ms=dict(zip(["project_count", "offsets", "lists", "raster_tensor", "raster_alu", "output_map"], stage_ms)),
                     cpu_baseline=cpu)
         print(json.dumps(line), flush=True)
     if world > 1:

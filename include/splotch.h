@@ -89,6 +89,8 @@ typedef struct {
 typedef enum { SPLOTCH_ADDITIVE = 0, SPLOTCH_ABSORB = 1 } splotch_mode;
 
 #define SPLOTCH_RAW_SUM 1u /* additive mode writes S_c = sum_p E_pc tau_p, not 1 - exp(-S_c)   */
+#define SPLOTCH_NO_TENSOR 2u /* additive mode: accumulate every pixel on the FP32 ALUs; by default the
+                              fully covered row segments of big splats run as split-TF32 tcgen05 MMAs */
 
 typedef struct {
     float brightness[SPLOTCH_MAX_TYPES];     /* scales E per type                             */
@@ -96,7 +98,7 @@ typedef struct {
     int32_t mode;                            /* splotch_mode                                  */
     float support_f;                         /* f of PAPER.md:69; > 0; the configs use 3      */
     float z_near;                            /* cull view-space depth <= z_near               */
-    uint32_t flags;                          /* SPLOTCH_RAW_SUM                               */
+    uint32_t flags;                          /* SPLOTCH_RAW_SUM | SPLOTCH_NO_TENSOR           */
 } splotch_params;
 
 /* ------------------------------------------------------------------------------------------
@@ -207,14 +209,15 @@ int splotch_debug_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp,
 
 /* Per-stage timing of splotch_render with CUDA events recorded on the caller's stream (used by
  * bench.py for the roofline of the dominant kernel).  splotch_profile_enable(1) resets the
- * record; while enabled every splotch_render records 6 events (up to 256 calls).
+ * record; while enabled every splotch_render records 7 events (up to 256 calls).
  * splotch_profile_read SYNCHRONISES on the last recorded event and returns the mean
- * milliseconds per call of the 5 stages: [0] transform/cull/colour + bin count (K1),
+ * milliseconds per call of the 6 stages: [0] transform/cull/colour + bin count (K1),
  * [1] offsets scan + work units, [2] lists (scatter, or depth sort + ordered split),
- * [3] tile rasteriser (K3), [4] output map / merge (K4).
+ * [3] tensor-core rasteriser (K3t; 0 in absorb mode and with SPLOTCH_NO_TENSOR),
+ * [4] ALU tile rasteriser (K3), [5] output map / merge (K4).
  * splotch_launch_count: kernels launched by this library in this process so far. */
 int splotch_profile_enable(int on);
-int splotch_profile_read(double *stage_ms /* host, 5 doubles */, int64_t *calls /* host */);
+int splotch_profile_read(double *stage_ms /* host, 6 doubles */, int64_t *calls /* host */);
 unsigned long long splotch_launch_count(void);
 
 const char *splotch_status_string(int status);

@@ -25,6 +25,7 @@ SPLOTCH_ERR_LIMIT = -4
 SPLOTCH_ADDITIVE = 0
 SPLOTCH_ABSORB = 1
 SPLOTCH_RAW_SUM = 1
+SPLOTCH_NO_TENSOR = 2
 
 # every symbol include/splotch.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
@@ -277,8 +278,8 @@ def splotch_profile_enable(on: bool) -> None:
 
 
 def splotch_profile_read():
-    """(list of 5 mean stage times in ms, number of profiled calls); synchronises."""
-    ms = (C.c_double * 5)()
+    """(list of 6 mean stage times in ms, number of profiled calls); synchronises."""
+    ms = (C.c_double * 6)()
     calls = C.c_int64(0)
     _check("splotch_profile_read", _lib().splotch_profile_read(ms, C.byref(calls)))
     return [float(v) for v in ms], int(calls.value)

@@ -16,7 +16,7 @@ unsigned long long g_launch_count = 0;
 // optional per-stage timing of splotch_render with CUDA events on the caller's stream
 // ---------------------------------------------------------------------------------------------
 namespace {
-constexpr int kStages = 5;          // project+count | offsets | lists | raster | output map
+constexpr int kStages = 6;          // project+count | offsets | lists | raster (tensor cores) | raster (ALU) | output map
 constexpr int kMaxProfiledCalls = 256;
 struct Profile {
     bool on = false;
@@ -365,11 +365,19 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
     if (rc) return rc;
     if (!absorb) SPLOTCH_CUDA_TRY(cudaMemsetAsync(out_rgb, 0, (size_t)n_values * 4, c.st));
     prof_mark(3, c.st);
+    if (absorb) prof_mark(4, c.st);
     if (!absorb) {
-        rc = launch_raster_additive(c.at<SplatAdd>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
-                                    c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
-        if (rc) return rc;
+        const int mma_on = (params->flags & SPLOTCH_NO_TENSOR) ? 0 : 1;
+        if (mma_on) {
+            rc = launch_raster_additive_mma(c.at<SplatAdd>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
+                                            c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
+            if (rc) return rc;
+        }
         prof_mark(4, c.st);
+        rc = launch_raster_additive(c.at<SplatAdd>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
+                                    c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), mma_on, c.st);
+        if (rc) return rc;
+        prof_mark(5, c.st);
         if (!(params->flags & SPLOTCH_RAW_SUM)) {
             rc = launch_normalize(out_rgb, out_rgb, n_values, c.st);
             if (rc) return rc;
@@ -378,7 +386,7 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
         rc = launch_raster_absorb(c.at<SplatAbs>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
                                   c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, c.at<float>(c.L.partials), c.head(), c.st);
         if (rc) return rc;
-        prof_mark(4, c.st);
+        prof_mark(5, c.st);
         rc = launch_merge_absorb(c.at<float>(c.L.partials), c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
         if (rc) return rc;
     }

@@ -86,6 +86,7 @@ finish_offsets_kernel(const uint32_t *__restrict__ bin_count, const uint64_t *__
         head->pairs = D;
         head->n_units = 0;
         head->work_counter = 0;
+        head->mma_counter = 0;
         if (D > max_pairs) head->status = -2;   // SPLOTCH_ERR_WORKSPACE
     }
     __syncthreads();

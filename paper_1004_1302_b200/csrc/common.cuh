@@ -80,7 +80,8 @@ struct WorkHead {
     unsigned long long updates;     // debug_stats: (particle, covered pixel) updates
     uint32_t work_counter;          // persistent-kernel ticket
     uint32_t scan_ticket;           // decoupled look-back tile ticket
-    uint32_t pad[6];
+    uint32_t mma_counter;           // ticket of the tensor-core rasteriser
+    uint32_t pad[5];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -159,7 +160,11 @@ constexpr uint32_t kChunkAdd = 2048;   // splats per additive work unit
 constexpr uint32_t kChunkAbs = 4096;   // splats per absorb work unit
 int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                           WorkHead *head, cudaStream_t st);
+                           WorkHead *head, int mma_on, cudaStream_t st);
+// raster_mma.cu: the fully covered row segments of the additive mode on the tensor cores
+int launch_raster_additive_mma(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
+                               const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
+                               WorkHead *head, cudaStream_t st);
 int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const uint64_t *bin_offset,
                          const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam,
                          float *partials, WorkHead *head, cudaStream_t st);

@@ -39,6 +39,9 @@ struct SmemAdd {
 };
 
 // one (splat, tile) pair: this lane's 8 pixels of row `y` of the tile, channels packed as f32x2
+// The row record's fourth word is the coverage threshold thr / gy with two flags folded in: its
+// sign bit says "segment 0 of this row is handled by the tensor-core kernel", its lowest mantissa
+// bit the same for segment 1 (raster_common.cuh: seg_handled); a handled segment contributes 0 here.
 template <bool kRim>
 __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const float4 *__restrict__ rows, int x, int y,
                                            float2 (&acc)[3][4])
@@ -48,10 +51,13 @@ __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const 
     const float4 r = rows[y];
     float2 p[4] = { make_float2(g0.x, g0.y), make_float2(g0.z, g0.w), make_float2(g1.x, g1.y), make_float2(g1.z, g1.w) };
     if (kRim) {
+        const uint32_t wb = __float_as_uint(r.w);
+        const bool handled = (x & kSegPx) ? (wb & 1u) != 0u : (wb >> 31) != 0u;
+        const float T = handled ? __int_as_float(0x7f800000) : fabsf(r.w);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            p[q].x = p[q].x >= r.w ? p[q].x : 0.0f;
-            p[q].y = p[q].y >= r.w ? p[q].y : 0.0f;
+            p[q].x = p[q].x >= T ? p[q].x : 0.0f;
+            p[q].y = p[q].y >= T ? p[q].y : 0.0f;
         }
     }
     const float2 wr = make_float2(r.x, r.x), wg = make_float2(r.y, r.y), wb = make_float2(r.z, r.z);
@@ -66,7 +72,7 @@ __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const 
 __global__ void __launch_bounds__(kRasThreads, 2)
 raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
                        const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
-                       int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok)
+                       int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok, int mma_on)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SmemAdd &sm = *reinterpret_cast<SmemAdd *>(smem_raw);
@@ -110,40 +116,70 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
             }
             cp_async_commit();
         };
-        // 8 threads per splat: each 8 gx values, 8 row records and the class of two tiles
+        // 8 threads per splat: each 8 gx values, 8 row records and the class of two tiles.  Every lane
+        // runs the whole body (slots without a splat work on a zero record) because the split between
+        // this kernel and the tensor-core kernel is agreed on with warp shuffles.
         auto produce = [&](int b, int slot) {
             const int s = tid >> 3, part = tid & 7;
             const uint32_t e = (uint32_t)b * kBatch + s;
-            if (b >= n_batches || e >= count) {
-                *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = 0;
-                return;
+            const bool valid = b < n_batches && e < count;
+            float4 g = make_float4(0.f, 0.f, 0.f, 0.f), a = g;
+            if (valid) {
+                g = *reinterpret_cast<const float4 *>(&sm.rec[slot][s]);        // sx, sy, c, R
+                a = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 1);  // a_r, a_g, a_b, bins
             }
-            const float4 g = *reinterpret_cast<const float4 *>(&sm.rec[slot][s]);        // sx, sy, c, R
-            const float4 a = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 1);  // a_r, a_g, a_b, bins
+            float4 v[2];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {           // columns part*4 + 32h .. +3: conflict-free 128-bit stores
-                const float x0 = (float)(px0 + part * 4 + 32 * h) + 0.5f;
-                float4 v;
-                float t;
-                t = (x0 - g.x) * g.z;          v.x = ex2_approx(-t * t);
-                t = (x0 + 1.0f - g.x) * g.z;   v.y = ex2_approx(-t * t);
-                t = (x0 + 2.0f - g.x) * g.z;   v.z = ex2_approx(-t * t);
-                t = (x0 + 3.0f - g.x) * g.z;   v.w = ex2_approx(-t * t);
-                *reinterpret_cast<float4 *>(&sm.gx[slot][s][part * 4 + 32 * h]) = v;
+                const int c0 = px0 + part * 4 + 32 * h;
+                v[h].x = gauss1d(pixel_centre(c0), g.x, g.z);
+                v[h].y = gauss1d(pixel_centre(c0 + 1), g.x, g.z);
+                v[h].z = gauss1d(pixel_centre(c0 + 2), g.x, g.z);
+                v[h].w = gauss1d(pixel_centre(c0 + 3), g.x, g.z);
+                *reinterpret_cast<float4 *>(&sm.gx[slot][s][part * 4 + 32 * h]) = v[h];
             }
+            // segments handled by the tensor-core kernel (same predicate, same bits: raster_common.cuh)
+            unsigned adm = 0u;
+            float m0 = -1.0f, m1 = -1.0f;
+            if (mma_on) {
+                const int first = lane & ~7, last = first + 7;
+                m0 = fminf(__shfl_sync(0xffffffffu, v[0].x, first), __shfl_sync(0xffffffffu, v[0].w, last));
+                m1 = fminf(__shfl_sync(0xffffffffu, v[1].x, first), __shfl_sync(0xffffffffu, v[1].w, last));
+                if (valid) adm = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+            }
+            unsigned hb0 = 0u, hb1 = 0u;            // bit k: row part + 8k handled in segment 0 / 1
 #pragma unroll
             for (int k = 0; k < 8; ++k) {           // rows part + 8k
                 const int j = part + 8 * k;
-                const float t = ((float)(py0 + j) + 0.5f - g.y) * g.z;
-                const float gy = ex2_approx(-t * t);
-                sm.row[slot][s][j] = make_float4(a.x * gy, a.y * gy, a.z * gy, __fdividef(thr, gy));
+                const float gy = gauss1d(pixel_centre(py0 + j), g.y, g.z);
+                const float T = row_threshold(thr, gy);
+                const unsigned hd = seg_handled(adm, m0, m1, T);
+                hb0 |= (hd & 1u) << k;
+                hb1 |= (hd >> 1) << k;
+                const uint32_t w = (__float_as_uint(T) & 0x7ffffffeu) | ((hd & 1u) << 31) | (hd >> 1);
+                sm.row[slot][s][j] = make_float4(a.x * gy, a.y * gy, a.z * gy, __uint_as_float(w));
+            }
+            unsigned all0 = hb0, all1 = hb1, any0 = hb0, any1 = hb1;
+            if (mma_on) {
+#pragma unroll
+                for (int d = 1; d < 8; d <<= 1) {
+                    all0 &= __shfl_xor_sync(0xffffffffu, all0, d);
+                    all1 &= __shfl_xor_sync(0xffffffffu, all1, d);
+                    any0 |= __shfl_xor_sync(0xffffffffu, any0, d);
+                    any1 |= __shfl_xor_sync(0xffffffffu, any1, d);
+                }
             }
             unsigned short c2 = 0;
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 const int t = 2 * part + k;
                 const int tpx = px0 + (t & 3) * kTilePx, tpy = py0 + (t >> 2) * kTilePx;
-                c2 |= (unsigned short)(classify_tile(g.x, g.y, g.w, (float)tpx + 0.5f, (float)tpy + 0.5f, W, H, tpx, tpy) << (8 * k));
+                int cl = valid ? classify_tile(g.x, g.y, g.w, (float)tpx + 0.5f, (float)tpy + 0.5f, W, H, tpx, tpy) : 0;
+                const unsigned rows2 = 3u << (2 * (t >> 2));           // the tile's 16 rows are bits 2ty, 2ty+1 of every part
+                const unsigned all = (t & 2) ? all1 : all0, any = (t & 2) ? any1 : any0;
+                if ((all & rows2) == rows2) cl = 0;                    // every row of the tile is done on the tensor cores
+                else if ((any & rows2) && cl == 2) cl = 1;             // some rows are: take the masking path
+                c2 |= (unsigned short)(cl << (8 * k));
             }
             *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = c2;
         };
@@ -232,7 +268,7 @@ normalize_kernel(const float *__restrict__ S, float *__restrict__ out, long long
 
 int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                           WorkHead *head, cudaStream_t st)
+                           WorkHead *head, int mma_on, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
@@ -242,7 +278,7 @@ int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const 
     }
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
     raster_additive_kernel<<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(
-        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok);
+        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, mma_on);
     SPLOTCH_LAUNCH_CHECK();
     return 0;
 }

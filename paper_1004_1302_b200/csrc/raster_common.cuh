@@ -40,10 +40,49 @@ __device__ __forceinline__ int classify_tile(float sx, float sy, float R, float 
     const float x_hi = x_lo + (tw - 1.0f), y_hi = y_lo + (th - 1.0f);
     const float nx = fmaxf(fmaxf(x_lo - sx, sx - x_hi), 0.0f), ny = fmaxf(fmaxf(y_lo - sy, sy - y_hi), 0.0f);
     const float fx = fmaxf(sx - x_lo, x_hi - sx), fy = fmaxf(sy - y_lo, y_hi - sy);
-    const float R2 = R * R;
-    if (nx * nx + ny * ny > R2 * 1.00001f) return 0;
-    if (fx * fx + fy * fy < R2 * 0.99999f) return 2;
+    const float R2 = __fmul_rn(R, R);
+    if (__fmaf_rn(nx, nx, __fmul_rn(ny, ny)) > __fmul_rn(R2, 1.00001f)) return 0;
+    if (__fmaf_rn(fx, fx, __fmul_rn(fy, fy)) < __fmul_rn(R2, 0.99999f)) return 2;
     return 1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Split of the additive work between the tensor-core kernel (raster_mma.cu) and the ALU kernel
+// (raster_add.cu).  A 64x64 block has two column groups g (32 pixels each); the row segment
+// (row j, group g) of a splat is HANDLED by the tensor-core kernel when the splat is admitted
+// for g and both end pixels of the segment pass the coverage test (the circle is convex, so
+// every pixel between them passes too).  Both kernels evaluate the functions below on the same
+// record words; every operation is an explicitly rounded intrinsic or a single hardware
+// approximation, so the two kernels take bit-identical decisions and every covered pixel is
+// accumulated exactly once.
+// ---------------------------------------------------------------------------------------------
+constexpr int kSegPx = 32;
+
+__device__ __forceinline__ float pixel_centre(int p) { return __fadd_rn((float)p, 0.5f); }
+
+// exp(-((x - s) / sigma)^2) with c = sqrt(log2 e) / sigma
+__device__ __forceinline__ float gauss1d(float x, float s, float c)
+{
+    const float t = __fmul_rn(__fsub_rn(x, s), c);
+    return ex2_approx(-__fmul_rn(t, t));
+}
+
+// coverage threshold on gx for a row whose factor is gy:  gx * gy >= thr  <=>  gx >= thr / gy
+__device__ __forceinline__ float row_threshold(float thr, float gy) { return __fdividef(thr, gy); }
+
+// bit g set: the splat has (at the row nearest to its centre) a fully covered segment in group g.
+// m0 / m1 = min of gx over the two end pixels of segment 0 / 1.
+__device__ __forceinline__ unsigned seg_admit(float sy, float c, float R, float thr, int py0, float m0, float m1)
+{
+    if (!(R >= 15.5f)) return 0u;                      // half chord of a 32-pixel segment
+    const float jf = fminf(fmaxf(floorf(__fsub_rn(sy, (float)py0)), 0.0f), (float)(kBlockPx - 1));
+    const float T = row_threshold(thr, gauss1d(__fadd_rn(__fadd_rn((float)py0, jf), 0.5f), sy, c));
+    return (m0 >= T ? 1u : 0u) | (m1 >= T ? 2u : 0u);
+}
+
+__device__ __forceinline__ unsigned seg_handled(unsigned adm, float m0, float m1, float T)
+{
+    return adm & ((m0 >= T ? 1u : 0u) | (m1 >= T ? 2u : 0u));
 }
 
 struct UnitInfo {

@@ -1,0 +1,379 @@
+// raster_mma.cu -- K3t: the interior of big splats on the 5th-generation tensor cores (step a8).
+//
+// In the additive mode (A = E) a pixel of a 64x64 block receives
+//     S_c(i, j) = sum_p  a_{p,c} * gx_p(i) * gy_p(j) * [pixel (i, j) inside the truncation circle of p],
+// gx_p(i) = exp(-(i + 1/2 - sx_p)^2 / sigma_p^2), gy_p(j) likewise (the Gaussian of PAPER.md:69 is
+// separable).  Wherever the indicator is 1 for a whole 32-pixel row segment this is a sum of rank-1
+// updates, i.e. a dense contraction over the splat index p:
+//     D_g[(c, i), j] = sum_p  A_g[(c, i), p] * B_g[p, j],
+//     A_g[(c, i), p] = a_{p,c} gx_p(32 g + i)            (128 rows: 3 channels x 32 columns, 32 rows of padding)
+//     B_g[p, j]      = gy_p(j) * handled(p, j, g)        (64 columns: the rows of the block)
+// with g = 0, 1 the two column groups of the block.  handled(p, j, g) (raster_common.cuh) is 1 when
+// the whole segment lies inside the circle; the remaining (rim) pixels are accumulated by the ALU
+// kernel of raster_add.cu, which evaluates the same predicate bit for bit and skips what is done here.
+//
+// The contraction runs as tcgen05.mma kind::tf32 (M = 128, N = 64, K = 8) with A in tensor memory
+// (written by the producing warps with tcgen05.st), B in shared memory (K-major, no swizzle) and the
+// fp32 accumulators D_0, D_1 in tensor memory.  Precision: every operand is split into two TF32 numbers
+// (hi = rna(v), lo = rna(v - hi)) and three products are accumulated (hi*hi + lo*hi + hi*lo), which
+// leaves a relative error of ~2^-21 per term instead of 2^-11 -- fp32 class, inside the 1e-4 parity
+// tolerance for any amplitude.
+//
+// One CTA (8 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
+// kUnitsPerTicket consecutive work units of its splat list:
+//   filter   : one thread per list entry tests seg_admit() and appends admitted splats to a ring queue;
+//   batch    : 16 queued splats; warps 0-2 / 4-6 (channel = warp & 3, group = warp >> 2) produce A,
+//              warps 3 and 7 produce B (one block row per lane); double buffered, so the MMAs of batch
+//              b run while batch b + 1 is produced; completion is tracked with tcgen05.commit -> mbarrier;
+//   flush    : tcgen05.ld of D, transposed through shared memory, vector red.global.add into the raw
+//              image (any summation order is legal when A = E).
+#include "raster_common.cuh"
+
+namespace splotch {
+
+namespace {
+
+constexpr int kMmaThreads = 256;
+constexpr int kMmaBatch = 16;             // splats per batch = two K = 8 steps
+constexpr int kQueue = 512;               // ring of admitted splats (power of two)
+constexpr int kFilterChunk = 256;         // list entries per filter pass (one per thread)
+constexpr int kUnitsPerTicket = 4;
+constexpr int kTmemCols = 256;
+constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
+constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
+
+struct SmemMma {
+    union {
+        struct {
+            float B[2][2][2][kMmaBatch * kBlockPx];          // [buf][g][hi | lo][((p / 4) * 64 + j) * 4 + p % 4]
+            float q_sx[kQueue], q_sy[kQueue], q_c[kQueue];
+            float q_a[3][kQueue];
+            float q_m[2][kQueue];                            // min end-pixel gx of group g, or -1 when not admitted
+        } w;
+        float stage[kBlockPx][kBlockPx * 3];                 // flush only
+    };
+    unsigned long long bar_free[2];
+    uint32_t tmem_base;
+    uint32_t q_tail;
+    uint32_t ticket;
+    UnitInfo unit;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ uint32_t tf32_rna(float v)
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
+    return r;
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    const uint32_t a = smem_u32(bar);
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+    }
+}
+
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                   "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+                 : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+                   "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// D[tmem d] (+)= A[tmem a] (128 x 8 tf32) * B[smem descriptor] (8 x 64 tf32)
+__device__ __forceinline__ void mma_tf32_ts(uint32_t d, uint32_t a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d), "r"(a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+// K-major, no swizzle: 16-byte units ((8, n), 2) : ((1, SBO), LBO); here [k / 4][j][k % 4] floats
+__device__ __forceinline__ uint64_t b_descriptor(const float *b)
+{
+    const uint64_t lbo = (uint64_t)(kBlockPx * 16) >> 4, sbo = 128 >> 4;
+    return (uint64_t)((smem_u32(b) >> 4) & 0x3FFFu) | (lbo << 16) | (sbo << 32) | (1ull << 46);
+}
+
+constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kBlockPx >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+
+__global__ void __launch_bounds__(kMmaThreads, 2)
+raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
+                           const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
+                           int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SmemMma &sm = *reinterpret_cast<SmemMma *>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int quarter = warp & 3, grp = warp >> 2;       // TMEM lane quarter (= channel for quarter < 3), column group
+    const uint32_t n_units = head->n_units;
+
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(kTmemCols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.bar_free[0])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.bar_free[1])));
+        asm volatile("fence.mbarrier_init.release.cluster;");
+        sm.q_tail = 0;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = sm.tmem_base;
+    const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
+    if (warp == 3) {                                      // rows 96..127 of A are padding: zero them once
+        uint32_t z[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) z[k] = 0u;
+#pragma unroll
+        for (int c0 = 0; c0 < 128; c0 += 16) tmem_st16(lane_addr + kACol + c0, z);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+
+    uint32_t uses[2] = { 0u, 0u };                        // commits issued on bar_free[buf]
+    uint32_t n_batches = 0;                               // batches issued so far (buffer = parity)
+    uint32_t q_head = 0;
+    bool fresh = true;                                    // D holds nothing yet: the first MMAs overwrite it
+    int px0 = 0, py0 = 0;
+
+    // ---- one batch of 16 queued splats: produce A (TMEM) and B (smem), then issue 12 MMAs ----
+    auto process_batch = [&]() {
+        const uint32_t buf = n_batches & 1u;
+        if (uses[buf] > 0) mbar_wait(&sm.bar_free[buf], (uses[buf] - 1u) & 1u);     // MMAs that read this buffer are done
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        if (quarter < 3) {
+            const float x = pixel_centre(px0 + kSegPx * grp + lane);
+            uint32_t hi[16], lo[16];
+#pragma unroll
+            for (int k = 0; k < kMmaBatch; ++k) {
+                const uint32_t s = (q_head + k) & (kQueue - 1);
+                const float v = __fmul_rn(sm.w.q_a[quarter][s], gauss1d(x, sm.w.q_sx[s], sm.w.q_c[s]));
+                hi[k] = tf32_rna(v);
+                lo[k] = tf32_rna(__fsub_rn(v, __uint_as_float(hi[k])));
+            }
+            const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
+            tmem_st16(a, hi);
+            tmem_st16(a + 16, lo);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        } else {
+            const int j = grp * 32 + lane;
+            const float y = pixel_centre(py0 + j);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                float bh[2][4], bl[2][4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t s = (q_head + 4 * q + k) & (kQueue - 1);
+                    const float gy = gauss1d(y, sm.w.q_sy[s], sm.w.q_c[s]);
+                    const float T = row_threshold(thr, gy);
+                    const float ghi = __uint_as_float(tf32_rna(gy));
+                    const float glo = __uint_as_float(tf32_rna(__fsub_rn(gy, ghi)));
+                    const bool h0 = sm.w.q_m[0][s] >= T, h1 = sm.w.q_m[1][s] >= T;
+                    bh[0][k] = h0 ? ghi : 0.0f;  bl[0][k] = h0 ? glo : 0.0f;
+                    bh[1][k] = h1 ? ghi : 0.0f;  bl[1][k] = h1 ? glo : 0.0f;
+                }
+                const int at = (q * kBlockPx + j) * 4;
+#pragma unroll
+                for (int g = 0; g < 2; ++g) {
+                    *reinterpret_cast<float4 *>(&sm.w.B[buf][g][0][at]) = make_float4(bh[g][0], bh[g][1], bh[g][2], bh[g][3]);
+                    *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0], bl[g][1], bl[g][2], bl[g][3]);
+                }
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncthreads();
+        if (tid == kMmaThreads - 32) {                    // lane 0 of warp 7 issues for the CTA
+            asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                const uint32_t d = tmem + kDCol + g * 64;
+                const uint64_t b_hi = b_descriptor(sm.w.B[buf][g][0]), b_lo = b_descriptor(sm.w.B[buf][g][1]);
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    const uint32_t a_hi = tmem + kACol + buf * 64 + g * 32 + 8 * s, a_lo = a_hi + 16;
+                    const uint64_t step = (uint64_t)((8 * kBlockPx * 4) >> 4) * s;      // two 16-byte K chunks per step
+                    mma_tf32_ts(d, a_hi, b_hi + step, kIdesc, (fresh && s == 0) ? 0u : 1u);
+                    mma_tf32_ts(d, a_lo, b_hi + step, kIdesc, 1u);
+                    mma_tf32_ts(d, a_hi, b_lo + step, kIdesc, 1u);
+                }
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                         ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
+        }
+        uses[buf] += 1u;
+        n_batches += 1u;
+        q_head += kMmaBatch;
+        fresh = false;
+    };
+
+    // ---- pad the queue to a whole batch and run it ----
+    auto drain = [&]() {
+        __syncthreads();
+        const uint32_t tail = sm.q_tail;
+        const uint32_t rem = tail - q_head;
+        if (rem == 0) return;
+        const uint32_t pad = kMmaBatch - rem;
+        if ((uint32_t)tid < pad) {
+            const uint32_t s = (tail + tid) & (kQueue - 1);
+            sm.w.q_sx[s] = 0.0f; sm.w.q_sy[s] = 0.0f; sm.w.q_c[s] = 0.0f;
+            sm.w.q_a[0][s] = 0.0f; sm.w.q_a[1][s] = 0.0f; sm.w.q_a[2][s] = 0.0f;
+            sm.w.q_m[0][s] = -1.0f; sm.w.q_m[1][s] = -1.0f;
+        }
+        __syncthreads();
+        if (tid == 0) sm.q_tail = tail + pad;
+        process_batch();
+    };
+
+    // ---- wait for every MMA, add D to the raw image ----
+    auto flush = [&]() {
+        if (fresh) return;
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+            if (uses[b] > 0) mbar_wait(&sm.bar_free[b], (uses[b] - 1u) & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        __syncthreads();                                  // B and the queue are dead: the stage may overwrite them
+        if (quarter < 3) {
+#pragma unroll
+            for (int c0 = 0; c0 < kBlockPx; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16(lane_addr + kDCol + grp * 64 + c0, v);
+#pragma unroll
+                for (int q = 0; q < 16; ++q) sm.stage[c0 + q][(kSegPx * grp + lane) * 3 + quarter] = __uint_as_float(v[q]);
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncthreads();
+        const bool vec = vec_ok && px0 + kBlockPx <= W;
+        for (int idx = tid; idx < kBlockPx * (kBlockPx * 3 / 4); idx += kMmaThreads) {
+            const int row = idx / (kBlockPx * 3 / 4), q4 = idx % (kBlockPx * 3 / 4);
+            const int Y = py0 + row;
+            if (Y >= H) continue;
+            const float4 v = *reinterpret_cast<const float4 *>(&sm.stage[row][4 * q4]);
+            float *dst = S + ((size_t)Y * W + px0) * 3;
+            if (vec) {
+                red_add_v4(dst + 4 * q4, v.x, v.y, v.z, v.w);
+            } else {
+                const float e[4] = { v.x, v.y, v.z, v.w };
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int f = 4 * q4 + k;
+                    if (px0 + f / 3 < W) atomicAdd(dst + f, e[k]);
+                }
+            }
+        }
+        __syncthreads();
+        fresh = true;
+    };
+
+    while (true) {
+        if (tid == 0) sm.ticket = atomicAdd(&head->mma_counter, 1u);
+        __syncthreads();
+        const uint32_t u0 = sm.ticket * kUnitsPerTicket;
+        if (u0 >= n_units) break;
+        const uint32_t u1 = min(u0 + (uint32_t)kUnitsPerTicket, n_units);
+        int cur_bin = -1;
+        for (uint32_t u = u0; u < u1; ++u) {
+            __syncthreads();
+            if (tid == 0) {
+                const int b = find_bin(unit_prefix, n_bins, u);
+                const unsigned long long lo = bin_offset[b] + (unsigned long long)(u - unit_prefix[b]) * kChunkAdd;
+                const unsigned long long rest = bin_offset[b + 1] - lo;
+                sm.unit.bin = b;
+                sm.unit.first = lo;
+                sm.unit.count = (uint32_t)(rest < kChunkAdd ? rest : kChunkAdd);
+            }
+            __syncthreads();
+            const int bin = sm.unit.bin;
+            const uint32_t count = sm.unit.count;
+            const unsigned long long first = sm.unit.first;
+            if (bin != cur_bin) {
+                if (cur_bin >= 0) { drain(); flush(); }
+                cur_bin = bin;
+                px0 = (bin % nbx) * kBlockPx;
+                py0 = (bin / nbx) * kBlockPx;
+            }
+            for (uint32_t off = 0; off < count; off += kFilterChunk) {
+                // filter: one list entry per thread
+                bool adm = false;
+                float4 geo = make_float4(0.f, 0.f, 0.f, 0.f);
+                float m0 = -1.0f, m1 = -1.0f;
+                uint32_t id = 0;
+                if (off + tid < count) {
+                    id = __ldg(list + first + off + tid);
+                    geo = __ldg(reinterpret_cast<const float4 *>(records + id));
+                    if (geo.w >= 15.5f) {
+                        const float e0 = gauss1d(pixel_centre(px0), geo.x, geo.z);
+                        const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), geo.x, geo.z);
+                        const float e2 = gauss1d(pixel_centre(px0 + kSegPx), geo.x, geo.z);
+                        const float e3 = gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), geo.x, geo.z);
+                        m0 = fminf(e0, e1);
+                        m1 = fminf(e2, e3);
+                        const unsigned a = seg_admit(geo.y, geo.z, geo.w, thr, py0, m0, m1);
+                        adm = a != 0u;
+                        if (!(a & 1u)) m0 = -1.0f;
+                        if (!(a & 2u)) m1 = -1.0f;
+                    }
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, adm);
+                uint32_t base = 0;
+                if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (adm) {
+                    const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
+                    const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
+                    sm.w.q_sx[s] = geo.x; sm.w.q_sy[s] = geo.y; sm.w.q_c[s] = geo.z;
+                    sm.w.q_a[0][s] = amp.x; sm.w.q_a[1][s] = amp.y; sm.w.q_a[2][s] = amp.z;
+                    sm.w.q_m[0][s] = m0; sm.w.q_m[1][s] = m1;
+                }
+                __syncthreads();
+                const uint32_t tail = sm.q_tail;
+                while (tail - q_head >= (uint32_t)kMmaBatch) process_batch();
+            }
+        }
+        drain();
+        flush();
+    }
+
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
+}
+
+}  // namespace
+
+int launch_raster_additive_mma(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
+                               const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
+                               WorkHead *head, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)sizeof(SmemMma)));
+        attr_set = true;
+    }
+    const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
+    raster_additive_mma_kernel<<<sm_count() * 2, kMmaThreads, sizeof(SmemMma), st>>>(
+        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok);
+    SPLOTCH_LAUNCH_CHECK();
+    return 0;
+}
+
+}  // namespace splotch

@@ -324,7 +324,7 @@ def test_repeat_calls_and_orbit_cameras(B):
         if j == 0:
             first = out
     again = sc.render(cam=w.cameras[0], raw=True).cpu().numpy()
-    np.testing.assert_allclose(again, first, rtol=2e-6, atol=1e-7)   # atomics: order of partial sums may differ
+    np.testing.assert_allclose(again, first, rtol=2e-5, atol=1e-6)   # atomics and MMA batching: order of partial sums may differ
 
 
 def test_stats_counts(B):
