@@ -139,13 +139,16 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                 *reinterpret_cast<float4 *>(&sm.gx[slot][s][part * 4 + 32 * h]) = v[h];
             }
             // segments handled by the tensor-core kernel (same predicate, same bits: raster_common.cuh)
-            unsigned adm = 0u;
+            unsigned adm = 0u, full = 0u;
             float m0 = -1.0f, m1 = -1.0f;
             if (mma_on) {
                 const int first = lane & ~7, last = first + 7;
                 m0 = fminf(__shfl_sync(0xffffffffu, v[0].x, first), __shfl_sync(0xffffffffu, v[0].w, last));
                 m1 = fminf(__shfl_sync(0xffffffffu, v[1].x, first), __shfl_sync(0xffffffffu, v[1].w, last));
-                if (valid) adm = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+                if (valid) {
+                    adm = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+                    full = seg_full(adm, g.y, g.z, thr, py0, m0, m1);
+                }
             }
             unsigned hb0 = 0u, hb1 = 0u;            // bit k: row part + 8k handled in segment 0 / 1
 #pragma unroll
@@ -153,7 +156,7 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                 const int j = part + 8 * k;
                 const float gy = gauss1d(pixel_centre(py0 + j), g.y, g.z);
                 const float T = row_threshold(thr, gy);
-                const unsigned hd = seg_handled(adm, m0, m1, T);
+                const unsigned hd = seg_handled(adm, full, m0, m1, gy, thr);
                 hb0 |= (hd & 1u) << k;
                 hb1 |= (hd >> 1) << k;
                 const uint32_t w = (__float_as_uint(T) & 0x7ffffffeu) | ((hd & 1u) << 31) | (hd >> 1);

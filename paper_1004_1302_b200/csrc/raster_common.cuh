@@ -67,23 +67,39 @@ __device__ __forceinline__ float gauss1d(float x, float s, float c)
     return ex2_approx(-__fmul_rn(t, t));
 }
 
-// coverage threshold on gx for a row whose factor is gy:  gx * gy >= thr  <=>  gx >= thr / gy
+// per-pixel coverage threshold of the ALU kernel on gx for a row whose factor is gy:  gx >= thr / gy
 __device__ __forceinline__ float row_threshold(float thr, float gy) { return __fdividef(thr, gy); }
 
-// bit g set: the splat has (at the row nearest to its centre) a fully covered segment in group g.
-// m0 / m1 = min of gx over the two end pixels of segment 0 / 1.
+// segment test: m = min of gx over the two end pixels of the segment, gy = factor of the row
+__device__ __forceinline__ bool seg_covered(float m, float gy, float thr) { return __fmul_rn(m, gy) >= thr; }
+
+// bit g set: the splat has (at the block row nearest to its centre) a fully covered segment in group g
 __device__ __forceinline__ unsigned seg_admit(float sy, float c, float R, float thr, int py0, float m0, float m1)
 {
     if (!(R >= 15.5f)) return 0u;                      // half chord of a 32-pixel segment
     const float jf = fminf(fmaxf(floorf(__fsub_rn(sy, (float)py0)), 0.0f), (float)(kBlockPx - 1));
-    const float T = row_threshold(thr, gauss1d(__fadd_rn(__fadd_rn((float)py0, jf), 0.5f), sy, c));
-    return (m0 >= T ? 1u : 0u) | (m1 >= T ? 2u : 0u);
+    const float gy = gauss1d(__fadd_rn(__fadd_rn((float)py0, jf), 0.5f), sy, c);
+    return (seg_covered(m0, gy, thr) ? 1u : 0u) | (seg_covered(m1, gy, thr) ? 2u : 0u);
 }
 
-__device__ __forceinline__ unsigned seg_handled(unsigned adm, float m0, float m1, float T)
+// bit g set: every row of the block is covered in group g (tested on the two extreme rows; the
+// circle is convex).  Part of the DEFINITION of "handled", so both kernels agree whatever the rounding.
+__device__ __forceinline__ unsigned seg_full(unsigned adm, float sy, float c, float thr, int py0, float m0, float m1)
 {
-    return adm & ((m0 >= T ? 1u : 0u) | (m1 >= T ? 2u : 0u));
+    if (adm == 0u) return 0u;
+    const float gy = fminf(gauss1d(pixel_centre(py0), sy, c), gauss1d(pixel_centre(py0 + kBlockPx - 1), sy, c));
+    return adm & ((seg_covered(m0, gy, thr) ? 1u : 0u) | (seg_covered(m1, gy, thr) ? 2u : 0u));
 }
+
+// bit g set: row segment (row with factor gy, group g) is accumulated by the tensor-core kernel
+__device__ __forceinline__ unsigned seg_handled(unsigned adm, unsigned full, float m0, float m1, float gy, float thr)
+{
+    return adm & (full | (seg_covered(m0, gy, thr) ? 1u : 0u) | (seg_covered(m1, gy, thr) ? 2u : 0u));
+}
+
+// The tensor-core kernel folds (adm, full) into the segment minima it queues: -1 never passes
+// seg_covered, kSegAlways always does (gy >= thr on the extreme rows of a full group).
+constexpr float kSegNever = -1.0f, kSegAlways = 1.0e30f;
 
 struct UnitInfo {
     int bin;

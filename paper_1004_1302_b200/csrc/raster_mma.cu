@@ -19,12 +19,18 @@
 // leaves a relative error of ~2^-21 per term instead of 2^-11 -- fp32 class, inside the 1e-4 parity
 // tolerance for any amplitude.
 //
-// One CTA (8 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
+// The split is computed with integer arithmetic on the fp32 bits (hi = (bits + 0x1000) & ~0x1fff, i.e.
+// round to nearest, ties away; lo = v - hi exactly; the tensor core ignores the 13 low bits of lo).
+//
+// One CTA (11 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
 // kUnitsPerTicket consecutive work units of its splat list:
-//   filter   : one thread per list entry tests seg_admit() and appends admitted splats to a ring queue;
-//   batch    : 16 queued splats; warps 0-2 / 4-6 (channel = warp & 3, group = warp >> 2) produce A,
-//              warps 3 and 7 produce B (one block row per lane); double buffered, so the MMAs of batch
-//              b run while batch b + 1 is produced; completion is tracked with tcgen05.commit -> mbarrier;
+//   filter   : one thread per list entry (ids and records prefetched one and two chunks ahead) tests
+//              seg_admit() and appends admitted splats to a ring queue in shared memory;
+//   batch    : 16 queued splats.  Warps 0-2 / 4-6 (channel = warp & 3, group = warp >> 2) produce A into
+//              tensor memory, warps 3, 7, 8, 9 produce B (32 block rows x 8 splats each), warp 10 issues
+//              the 12 MMAs of the batch.  Two buffers; producers -> issuer through an mbarrier `full`,
+//              issuer -> producers through tcgen05.commit on an mbarrier `free`; no CTA-wide barrier
+//              inside a filter chunk, so the MMAs of batch b run while batch b + 1 is produced;
 //   flush    : tcgen05.ld of D, transposed through shared memory, vector red.global.add into the raw
 //              image (any summation order is legal when A = E).
 #include "raster_common.cuh"
@@ -33,40 +39,37 @@ namespace splotch {
 
 namespace {
 
-constexpr int kMmaThreads = 256;
+constexpr int kMmaThreads = 352;          // 11 warps
+constexpr int kProducerWarps = 10;
+constexpr int kIssuerWarp = 10;
 constexpr int kMmaBatch = 16;             // splats per batch = two K = 8 steps
 constexpr int kQueue = 512;               // ring of admitted splats (power of two)
-constexpr int kFilterChunk = 256;         // list entries per filter pass (one per thread)
-constexpr int kUnitsPerTicket = 4;
+constexpr int kFilterChunk = 256;         // list entries per filter pass (one per thread of warps 0-7)
+constexpr int kUnitsPerTicket = 8;
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
 constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
+
+struct Range { int bin; uint32_t count; unsigned long long first; };
 
 struct SmemMma {
     union {
         struct {
             float B[2][2][2][kMmaBatch * kBlockPx];          // [buf][g][hi | lo][((p / 4) * 64 + j) * 4 + p % 4]
-            float q_sx[kQueue], q_sy[kQueue], q_c[kQueue];
-            float q_a[3][kQueue];
-            float q_m[2][kQueue];                            // min end-pixel gx of group g, or -1 when not admitted
+            float4 qA[3][kQueue];                            // per channel: sx, c, a_channel, -
+            float4 qB[kQueue];                               // sy, c, segment minimum of group 0, of group 1 (folded)
         } w;
         float stage[kBlockPx][kBlockPx * 3];                 // flush only
     };
-    unsigned long long bar_free[2];
+    unsigned long long bar_full[2], bar_free[2];
     uint32_t tmem_base;
     uint32_t q_tail;
     uint32_t ticket;
-    UnitInfo unit;
+    int n_ranges;
+    Range range[kUnitsPerTicket];
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ uint32_t tf32_rna(float v)
-{
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
-    return r;
-}
 
 __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
 {
@@ -76,6 +79,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(a), "r"(parity) : "memory");
     }
+}
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16])
@@ -112,6 +120,13 @@ __device__ __forceinline__ uint64_t b_descriptor(const float *b)
 
 constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kBlockPx >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 
+// v = hi + lo with hi a TF32 number (round to nearest, ties away) and lo = v - hi exact in fp32
+__device__ __forceinline__ void split_tf32(float v, uint32_t &hi, uint32_t &lo)
+{
+    hi = (__float_as_uint(v) + 0x1000u) & 0xffffe000u;
+    lo = __float_as_uint(__fsub_rn(v, __uint_as_float(hi)));
+}
+
 __global__ void __launch_bounds__(kMmaThreads, 2)
 raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
                            const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
@@ -120,7 +135,11 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SmemMma &sm = *reinterpret_cast<SmemMma *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int quarter = warp & 3, grp = warp >> 2;       // TMEM lane quarter (= channel for quarter < 3), column group
+    const int quarter = warp & 3, grp = (warp >> 2) & 1;   // TMEM lane quarter (= channel for quarter < 3), column group
+    const bool a_warp = warp < 8 && quarter < 3;
+    const bool b_warp = (warp < 8 && quarter == 3) || warp == 8 || warp == 9;
+    const int b_rows = warp == 3 ? 0 : warp == 7 ? 1 : warp == 8 ? 0 : 1;     // which 32 block rows
+    const int b_half = warp < 8 ? 0 : 1;                                      // which 8 splats of the batch
     const uint32_t n_units = head->n_units;
 
     if (warp == 0) {
@@ -128,8 +147,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.bar_free[0])));
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.bar_free[1])));
+        for (int b = 0; b < 2; ++b) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(&sm.bar_full[b])), "r"(kProducerWarps));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sm.bar_free[b])));
+        }
         asm volatile("fence.mbarrier_init.release.cluster;");
         sm.q_tail = 0;
     }
@@ -145,86 +166,94 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
 #pragma unroll
         for (int c0 = 0; c0 < 128; c0 += 16) tmem_st16(lane_addr + kACol + c0, z);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;");
     }
 
-    uint32_t uses[2] = { 0u, 0u };                        // commits issued on bar_free[buf]
-    uint32_t n_batches = 0;                               // batches issued so far (buffer = parity)
+    uint32_t uses0 = 0u, uses1 = 0u;                      // batches issued into buffer 0 / 1
+    uint32_t n_batches = 0;                               // batches so far (buffer = parity)
     uint32_t q_head = 0;
     bool fresh = true;                                    // D holds nothing yet: the first MMAs overwrite it
     int px0 = 0, py0 = 0;
 
-    // ---- one batch of 16 queued splats: produce A (TMEM) and B (smem), then issue 12 MMAs ----
-    auto process_batch = [&]() {
-        const uint32_t buf = n_batches & 1u;
-        if (uses[buf] > 0) mbar_wait(&sm.bar_free[buf], (uses[buf] - 1u) & 1u);     // MMAs that read this buffer are done
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        if (quarter < 3) {
-            const float x = pixel_centre(px0 + kSegPx * grp + lane);
-            uint32_t hi[16], lo[16];
+    // ---- nb batches of 16 queued splats; every role walks the same sequence ----
+    auto process_batches = [&](uint32_t nb) {
+        for (uint32_t it = 0; it < nb; ++it) {
+            const uint32_t buf = n_batches & 1u;
+            const uint32_t uses = buf ? uses1 : uses0;
+            if (warp == kIssuerWarp) {
+                if (lane == 0) {
+                    mbar_wait(&sm.bar_full[buf], uses & 1u);
+                    asm volatile("tcgen05.fence::after_thread_sync;");
 #pragma unroll
-            for (int k = 0; k < kMmaBatch; ++k) {
-                const uint32_t s = (q_head + k) & (kQueue - 1);
-                const float v = __fmul_rn(sm.w.q_a[quarter][s], gauss1d(x, sm.w.q_sx[s], sm.w.q_c[s]));
-                hi[k] = tf32_rna(v);
-                lo[k] = tf32_rna(__fsub_rn(v, __uint_as_float(hi[k])));
-            }
-            const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
-            tmem_st16(a, hi);
-            tmem_st16(a + 16, lo);
-            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-        } else {
-            const int j = grp * 32 + lane;
-            const float y = pixel_centre(py0 + j);
+                    for (int g = 0; g < 2; ++g) {
+                        const uint32_t d = tmem + kDCol + g * 64;
+                        const uint64_t b_hi = b_descriptor(sm.w.B[buf][g][0]), b_lo = b_descriptor(sm.w.B[buf][g][1]);
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                float bh[2][4], bl[2][4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const uint32_t s = (q_head + 4 * q + k) & (kQueue - 1);
-                    const float gy = gauss1d(y, sm.w.q_sy[s], sm.w.q_c[s]);
-                    const float T = row_threshold(thr, gy);
-                    const float ghi = __uint_as_float(tf32_rna(gy));
-                    const float glo = __uint_as_float(tf32_rna(__fsub_rn(gy, ghi)));
-                    const bool h0 = sm.w.q_m[0][s] >= T, h1 = sm.w.q_m[1][s] >= T;
-                    bh[0][k] = h0 ? ghi : 0.0f;  bl[0][k] = h0 ? glo : 0.0f;
-                    bh[1][k] = h1 ? ghi : 0.0f;  bl[1][k] = h1 ? glo : 0.0f;
+                        for (int s = 0; s < 2; ++s) {
+                            const uint32_t a_hi = tmem + kACol + buf * 64 + g * 32 + 8 * s, a_lo = a_hi + 16;
+                            const uint64_t step = (uint64_t)((8 * kBlockPx * 4) >> 4) * s;      // two 16-byte K chunks per step
+                            mma_tf32_ts(d, a_hi, b_hi + step, kIdesc, (fresh && s == 0) ? 0u : 1u);
+                            mma_tf32_ts(d, a_lo, b_hi + step, kIdesc, 1u);
+                            mma_tf32_ts(d, a_hi, b_lo + step, kIdesc, 1u);
+                        }
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                 ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
                 }
-                const int at = (q * kBlockPx + j) * 4;
+                __syncwarp();
+            } else {
+                if (uses > 0) mbar_wait(&sm.bar_free[buf], (uses - 1u) & 1u);     // the MMAs that read this buffer are done
+                if (a_warp) {
+                    asm volatile("tcgen05.fence::after_thread_sync;");
+                    const float x = pixel_centre(px0 + kSegPx * grp + lane);
+                    uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int g = 0; g < 2; ++g) {
-                    *reinterpret_cast<float4 *>(&sm.w.B[buf][g][0][at]) = make_float4(bh[g][0], bh[g][1], bh[g][2], bh[g][3]);
-                    *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0], bl[g][1], bl[g][2], bl[g][3]);
+                    for (int k = 0; k < kMmaBatch; ++k) {
+                        const float4 q = sm.w.qA[quarter][(q_head + k) & (kQueue - 1)];
+                        split_tf32(__fmul_rn(q.z, gauss1d(x, q.x, q.y)), hi[k], lo[k]);
+                    }
+                    const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
+                    tmem_st16(a, hi);
+                    tmem_st16(a + 16, lo);
+                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                    asm volatile("tcgen05.fence::before_thread_sync;");
+                } else {
+                    const int j = b_rows * 32 + lane;
+                    const float y = pixel_centre(py0 + j);
+#pragma unroll
+                    for (int qq = 0; qq < 2; ++qq) {
+                        const int q4 = 2 * b_half + qq;                           // group of 4 splats
+                        uint32_t bh[2][4], bl[2][4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const float4 q = sm.w.qB[(q_head + 4 * q4 + k) & (kQueue - 1)];
+                            const float gy = gauss1d(y, q.x, q.y);
+                            uint32_t ghi, glo;
+                            split_tf32(gy, ghi, glo);
+                            const bool h0 = seg_covered(q.z, gy, thr), h1 = seg_covered(q.w, gy, thr);
+                            bh[0][k] = h0 ? ghi : 0u;  bl[0][k] = h0 ? glo : 0u;
+                            bh[1][k] = h1 ? ghi : 0u;  bl[1][k] = h1 ? glo : 0u;
+                        }
+                        const int at = (q4 * kBlockPx + j) * 4;
+#pragma unroll
+                        for (int g = 0; g < 2; ++g) {
+                            *reinterpret_cast<uint4 *>(&sm.w.B[buf][g][0][at]) = make_uint4(bh[g][0], bh[g][1], bh[g][2], bh[g][3]);
+                            *reinterpret_cast<uint4 *>(&sm.w.B[buf][g][1][at]) = make_uint4(bl[g][0], bl[g][1], bl[g][2], bl[g][3]);
+                        }
+                    }
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&sm.bar_full[buf]);
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            if (buf) uses1 += 1u; else uses0 += 1u;
+            n_batches += 1u;
+            q_head += kMmaBatch;
+            fresh = false;
         }
-        asm volatile("tcgen05.fence::before_thread_sync;");
-        __syncthreads();
-        if (tid == kMmaThreads - 32) {                    // lane 0 of warp 7 issues for the CTA
-            asm volatile("tcgen05.fence::after_thread_sync;");
-#pragma unroll
-            for (int g = 0; g < 2; ++g) {
-                const uint32_t d = tmem + kDCol + g * 64;
-                const uint64_t b_hi = b_descriptor(sm.w.B[buf][g][0]), b_lo = b_descriptor(sm.w.B[buf][g][1]);
-#pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    const uint32_t a_hi = tmem + kACol + buf * 64 + g * 32 + 8 * s, a_lo = a_hi + 16;
-                    const uint64_t step = (uint64_t)((8 * kBlockPx * 4) >> 4) * s;      // two 16-byte K chunks per step
-                    mma_tf32_ts(d, a_hi, b_hi + step, kIdesc, (fresh && s == 0) ? 0u : 1u);
-                    mma_tf32_ts(d, a_lo, b_hi + step, kIdesc, 1u);
-                    mma_tf32_ts(d, a_hi, b_lo + step, kIdesc, 1u);
-                }
-            }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                         ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
-        }
-        uses[buf] += 1u;
-        n_batches += 1u;
-        q_head += kMmaBatch;
-        fresh = false;
     };
 
-    // ---- pad the queue to a whole batch and run it ----
+    // ---- pad the queue to a whole batch and run it (all threads; ends every range) ----
     auto drain = [&]() {
         __syncthreads();
         const uint32_t tail = sm.q_tail;
@@ -233,24 +262,22 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
         const uint32_t pad = kMmaBatch - rem;
         if ((uint32_t)tid < pad) {
             const uint32_t s = (tail + tid) & (kQueue - 1);
-            sm.w.q_sx[s] = 0.0f; sm.w.q_sy[s] = 0.0f; sm.w.q_c[s] = 0.0f;
-            sm.w.q_a[0][s] = 0.0f; sm.w.q_a[1][s] = 0.0f; sm.w.q_a[2][s] = 0.0f;
-            sm.w.q_m[0][s] = -1.0f; sm.w.q_m[1][s] = -1.0f;
+            sm.w.qA[0][s] = sm.w.qA[1][s] = sm.w.qA[2][s] = make_float4(0.f, 0.f, 0.f, 0.f);
+            sm.w.qB[s] = make_float4(0.f, 0.f, kSegNever, kSegNever);
         }
-        __syncthreads();
         if (tid == 0) sm.q_tail = tail + pad;
-        process_batch();
+        __syncthreads();
+        process_batches(1u);
     };
 
     // ---- wait for every MMA, add D to the raw image ----
     auto flush = [&]() {
         if (fresh) return;
-#pragma unroll
-        for (int b = 0; b < 2; ++b)
-            if (uses[b] > 0) mbar_wait(&sm.bar_free[b], (uses[b] - 1u) & 1u);
+        if (uses0 > 0) mbar_wait(&sm.bar_free[0], (uses0 - 1u) & 1u);
+        if (uses1 > 0) mbar_wait(&sm.bar_free[1], (uses1 - 1u) & 1u);
         asm volatile("tcgen05.fence::after_thread_sync;");
         __syncthreads();                                  // B and the queue are dead: the stage may overwrite them
-        if (quarter < 3) {
+        if (a_warp) {
 #pragma unroll
             for (int c0 = 0; c0 < kBlockPx; c0 += 16) {
                 uint32_t v[16];
@@ -258,8 +285,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
 #pragma unroll
                 for (int q = 0; q < 16; ++q) sm.stage[c0 + q][(kSegPx * grp + lane) * 3 + quarter] = __uint_as_float(v[q]);
             }
+            asm volatile("tcgen05.fence::before_thread_sync;");
         }
-        asm volatile("tcgen05.fence::before_thread_sync;");
         __syncthreads();
         const bool vec = vec_ok && px0 + kBlockPx <= W;
         for (int idx = tid; idx < kBlockPx * (kBlockPx * 3 / 4); idx += kMmaThreads) {
@@ -284,72 +311,90 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
     };
 
     while (true) {
-        if (tid == 0) sm.ticket = atomicAdd(&head->mma_counter, 1u);
+        // ---- ticket: kUnitsPerTicket consecutive work units = at most that many list ranges, one per bin ----
         __syncthreads();
-        const uint32_t u0 = sm.ticket * kUnitsPerTicket;
-        if (u0 >= n_units) break;
-        const uint32_t u1 = min(u0 + (uint32_t)kUnitsPerTicket, n_units);
-        int cur_bin = -1;
-        for (uint32_t u = u0; u < u1; ++u) {
-            __syncthreads();
-            if (tid == 0) {
+        if (tid == 0) {
+            const uint32_t t = atomicAdd(&head->mma_counter, 1u);
+            sm.ticket = t;
+            int nr = 0;
+            uint32_t u = t * kUnitsPerTicket;
+            const uint32_t u1 = min(u + (uint32_t)kUnitsPerTicket, n_units);
+            while (u < u1) {
                 const int b = find_bin(unit_prefix, n_bins, u);
                 const unsigned long long lo = bin_offset[b] + (unsigned long long)(u - unit_prefix[b]) * kChunkAdd;
-                const unsigned long long rest = bin_offset[b + 1] - lo;
-                sm.unit.bin = b;
-                sm.unit.first = lo;
-                sm.unit.count = (uint32_t)(rest < kChunkAdd ? rest : kChunkAdd);
+                const unsigned long long want = (unsigned long long)(u1 - u) * kChunkAdd, rest = bin_offset[b + 1] - lo;
+                const unsigned long long len = rest < want ? rest : want;
+                sm.range[nr].bin = b;
+                sm.range[nr].first = lo;
+                sm.range[nr].count = (uint32_t)len;
+                ++nr;
+                u += (uint32_t)((len + kChunkAdd - 1) / kChunkAdd);
             }
-            __syncthreads();
-            const int bin = sm.unit.bin;
-            const uint32_t count = sm.unit.count;
-            const unsigned long long first = sm.unit.first;
-            if (bin != cur_bin) {
-                if (cur_bin >= 0) { drain(); flush(); }
-                cur_bin = bin;
-                px0 = (bin % nbx) * kBlockPx;
-                py0 = (bin / nbx) * kBlockPx;
+            sm.n_ranges = nr;
+        }
+        __syncthreads();
+        if (sm.ticket * (uint32_t)kUnitsPerTicket >= n_units) break;
+        const int n_ranges = sm.n_ranges;
+        for (int r = 0; r < n_ranges; ++r) {
+            const int bin = sm.range[r].bin;
+            const uint32_t count = sm.range[r].count;
+            const unsigned long long first = sm.range[r].first;
+            px0 = (bin % nbx) * kBlockPx;
+            py0 = (bin / nbx) * kBlockPx;
+            // software-pipelined filter: ids two chunks ahead, records one chunk ahead
+            const bool filt = tid < kFilterChunk;
+            uint32_t id_cur = 0, id_next = 0;
+            float4 geo = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (filt) {
+                if ((uint32_t)tid < count) id_cur = __ldg(list + first + tid);
+                if ((uint32_t)tid + kFilterChunk < count) id_next = __ldg(list + first + kFilterChunk + tid);
+                if ((uint32_t)tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
             }
             for (uint32_t off = 0; off < count; off += kFilterChunk) {
-                // filter: one list entry per thread
-                bool adm = false;
-                float4 geo = make_float4(0.f, 0.f, 0.f, 0.f);
-                float m0 = -1.0f, m1 = -1.0f;
-                uint32_t id = 0;
-                if (off + tid < count) {
-                    id = __ldg(list + first + off + tid);
-                    geo = __ldg(reinterpret_cast<const float4 *>(records + id));
-                    if (geo.w >= 15.5f) {
-                        const float e0 = gauss1d(pixel_centre(px0), geo.x, geo.z);
-                        const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), geo.x, geo.z);
-                        const float e2 = gauss1d(pixel_centre(px0 + kSegPx), geo.x, geo.z);
-                        const float e3 = gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), geo.x, geo.z);
+                if (filt) {
+                    const float4 g = geo;
+                    const uint32_t id = id_cur;
+                    const bool have = off + tid < count;
+                    // prefetch for the next two chunks before the batches of this one
+                    id_cur = id_next;
+                    if (off + kFilterChunk + tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
+                    if (off + 2 * kFilterChunk + tid < count) id_next = __ldg(list + first + off + 2 * kFilterChunk + tid);
+                    bool adm = false;
+                    float m0 = kSegNever, m1 = kSegNever;
+                    if (have && g.w >= 15.5f) {
+                        const float e0 = gauss1d(pixel_centre(px0), g.x, g.z);
+                        const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), g.x, g.z);
+                        const float e2 = gauss1d(pixel_centre(px0 + kSegPx), g.x, g.z);
+                        const float e3 = gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), g.x, g.z);
                         m0 = fminf(e0, e1);
                         m1 = fminf(e2, e3);
-                        const unsigned a = seg_admit(geo.y, geo.z, geo.w, thr, py0, m0, m1);
+                        const unsigned a = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+                        const unsigned f = seg_full(a, g.y, g.z, thr, py0, m0, m1);
                         adm = a != 0u;
-                        if (!(a & 1u)) m0 = -1.0f;
-                        if (!(a & 2u)) m1 = -1.0f;
+                        m0 = (f & 1u) ? kSegAlways : (a & 1u) ? m0 : kSegNever;
+                        m1 = (f & 2u) ? kSegAlways : (a & 2u) ? m1 : kSegNever;
                     }
-                }
-                const unsigned bal = __ballot_sync(0xffffffffu, adm);
-                uint32_t base = 0;
-                if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (adm) {
-                    const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
-                    const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
-                    sm.w.q_sx[s] = geo.x; sm.w.q_sy[s] = geo.y; sm.w.q_c[s] = geo.z;
-                    sm.w.q_a[0][s] = amp.x; sm.w.q_a[1][s] = amp.y; sm.w.q_a[2][s] = amp.z;
-                    sm.w.q_m[0][s] = m0; sm.w.q_m[1][s] = m1;
+                    const unsigned bal = __ballot_sync(0xffffffffu, adm);
+                    uint32_t base = 0;
+                    if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (adm) {
+                        const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
+                        const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
+                        sm.w.qA[0][s] = make_float4(g.x, g.z, amp.x, 0.f);
+                        sm.w.qA[1][s] = make_float4(g.x, g.z, amp.y, 0.f);
+                        sm.w.qA[2][s] = make_float4(g.x, g.z, amp.z, 0.f);
+                        sm.w.qB[s] = make_float4(g.y, g.z, m0, m1);
+                    }
                 }
                 __syncthreads();
                 const uint32_t tail = sm.q_tail;
-                while (tail - q_head >= (uint32_t)kMmaBatch) process_batch();
+                process_batches((tail - q_head) / kMmaBatch);
+                __syncthreads();                          // every warp is done reading the queue before it is refilled
             }
+            drain();
+            flush();
         }
-        drain();
-        flush();
     }
 
     asm volatile("tcgen05.fence::before_thread_sync;");
