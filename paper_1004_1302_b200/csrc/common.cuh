@@ -47,6 +47,7 @@ struct RenderConst {
 // splat records written by the transform / cull / colour kernel (step a1-a3)
 // ---------------------------------------------------------------------------------------------
 constexpr uint32_t kInvisible = 0xFFFFFFFFu;
+constexpr uint32_t kListDone = 0x80000000u;   // pair-list flag set by the tensor-core kernel: no ALU work left (n < 2^31)
 
 struct __align__(16) SplatAdd {     // 32 B, additive mode
     float sx, sy;                   // screen position (pixels)
@@ -162,7 +163,7 @@ int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const 
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
                            WorkHead *head, int mma_on, cudaStream_t st);
 // raster_mma.cu: the fully covered row segments of the additive mode on the tensor cores
-int launch_raster_additive_mma(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
+int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const uint64_t *bin_offset,
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
                                WorkHead *head, cudaStream_t st);
 int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const uint64_t *bin_offset,

@@ -36,6 +36,7 @@ struct SmemAdd {
     unsigned char cls[2][kBatch][kTiles];
     UnitInfo unit;
     uint32_t unit_id;
+    uint32_t n_ids;
 };
 
 // one (splat, tile) pair: this lane's 8 pixels of row `y` of the tile, channels packed as f32x2
@@ -99,12 +100,25 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
         __syncthreads();
         if (sm.unit_id >= n_units) break;
         const int bin = sm.unit.bin;
-        const uint32_t count = sm.unit.count;
+        const uint32_t unit_count = sm.unit.count;
         const unsigned long long first = sm.unit.first;
         const int px0 = (bin % nbx) * kBlockPx, py0 = (bin / nbx) * kBlockPx;
 
-        for (uint32_t i = tid; i < count; i += kRasThreads) sm.ids[i] = __ldg(list + first + i);
+        // ids of the unit, without the entries the tensor-core kernel marked as finished
+        if (tid == 0) sm.n_ids = 0u;
         __syncthreads();
+        for (uint32_t i0 = 0; i0 < unit_count; i0 += kRasThreads) {
+            const uint32_t i = i0 + tid;
+            const uint32_t id = i < unit_count ? __ldg(list + first + i) : kListDone;
+            const bool keep = !(id & kListDone);
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            uint32_t base = 0;
+            if (lane == 0 && bal) base = atomicAdd(&sm.n_ids, (uint32_t)__popc(bal));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (keep) sm.ids[base + __popc(bal & ((1u << lane) - 1u))] = id;
+        }
+        __syncthreads();
+        const uint32_t count = sm.n_ids;
         const int n_batches = (int)((count + kBatch - 1) / kBatch);
 
         auto gather = [&](int b, int slot) {        // 64 threads copy 32 records of 32 B

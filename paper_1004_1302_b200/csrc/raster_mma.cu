@@ -25,7 +25,9 @@
 // One CTA (11 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
 // kUnitsPerTicket consecutive work units of its splat list:
 //   filter   : one thread per list entry (ids and records prefetched one and two chunks ahead) tests
-//              seg_admit() and appends admitted splats to a ring queue in shared memory;
+//              seg_admit() and appends admitted splats to a ring queue in shared memory; entries whose
+//              block is missed by the circle or entirely handled here get kListDone set in the list,
+//              so the ALU kernel (which runs next) drops them without fetching the record;
 //   batch    : 16 queued splats.  Warps 0-2 / 4-6 (channel = warp & 3, group = warp >> 2) produce A into
 //              tensor memory, warps 3, 7, 8, 9 produce B (32 block rows x 8 splats each), warp 10 issues
 //              the 12 MMAs of the batch.  Two buffers; producers -> issuer through an mbarrier `full`,
@@ -128,7 +130,7 @@ __device__ __forceinline__ void split_tf32(float v, uint32_t &hi, uint32_t &lo)
 }
 
 __global__ void __launch_bounds__(kMmaThreads, 2)
-raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
+raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__restrict__ list,
                            const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
                            int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok)
 {
@@ -206,10 +208,11 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
                 if (a_warp) {
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const float x = pixel_centre(px0 + kSegPx * grp + lane);
+                    const float4 *qa = &sm.w.qA[quarter][q_head & (kQueue - 1)];   // a batch never wraps: 16 | kQueue
                     uint32_t hi[16], lo[16];
 #pragma unroll
                     for (int k = 0; k < kMmaBatch; ++k) {
-                        const float4 q = sm.w.qA[quarter][(q_head + k) & (kQueue - 1)];
+                        const float4 q = qa[k];
                         split_tf32(__fmul_rn(q.z, gauss1d(x, q.x, q.y)), hi[k], lo[k]);
                     }
                     const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
@@ -220,13 +223,14 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
                 } else {
                     const int j = b_rows * 32 + lane;
                     const float y = pixel_centre(py0 + j);
+                    const float4 *qb = &sm.w.qB[q_head & (kQueue - 1)];
 #pragma unroll
                     for (int qq = 0; qq < 2; ++qq) {
                         const int q4 = 2 * b_half + qq;                           // group of 4 splats
                         uint32_t bh[2][4], bl[2][4];
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
-                            const float4 q = sm.w.qB[(q_head + 4 * q4 + k) & (kQueue - 1)];
+                            const float4 q = qb[4 * q4 + k];
                             const float gy = gauss1d(y, q.x, q.y);
                             uint32_t ghi, glo;
                             split_tf32(gy, ghi, glo);
@@ -346,8 +350,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
             uint32_t id_cur = 0, id_next = 0;
             float4 geo = make_float4(0.f, 0.f, 0.f, 0.f);
             if (filt) {
-                if ((uint32_t)tid < count) id_cur = __ldg(list + first + tid);
-                if ((uint32_t)tid + kFilterChunk < count) id_next = __ldg(list + first + kFilterChunk + tid);
+                if ((uint32_t)tid < count) id_cur = list[first + tid];
+                if ((uint32_t)tid + kFilterChunk < count) id_next = list[first + kFilterChunk + tid];
                 if ((uint32_t)tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
             }
             for (uint32_t off = 0; off < count; off += kFilterChunk) {
@@ -358,9 +362,16 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
                     // prefetch for the next two chunks before the batches of this one
                     id_cur = id_next;
                     if (off + kFilterChunk + tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
-                    if (off + 2 * kFilterChunk + tid < count) id_next = __ldg(list + first + off + 2 * kFilterChunk + tid);
+                    if (off + 2 * kFilterChunk + tid < count) id_next = list[first + off + 2 * kFilterChunk + tid];
                     bool adm = false;
                     float m0 = kSegNever, m1 = kSegNever;
+                    bool done = false;                     // nothing left for the ALU kernel in this block
+                    if (have) {                            // the circle misses the block (bins are pixel boxes: B-rules)
+                        const float x_lo = pixel_centre(px0), x_hi = pixel_centre(px0 + kBlockPx - 1);
+                        const float y_lo = pixel_centre(py0), y_hi = pixel_centre(py0 + kBlockPx - 1);
+                        const float nx = fmaxf(fmaxf(x_lo - g.x, g.x - x_hi), 0.0f), ny = fmaxf(fmaxf(y_lo - g.y, g.y - y_hi), 0.0f);
+                        done = __fmaf_rn(nx, nx, __fmul_rn(ny, ny)) > __fmul_rn(__fmul_rn(g.w, g.w), 1.00001f);
+                    }
                     if (have && g.w >= 15.5f) {
                         const float e0 = gauss1d(pixel_centre(px0), g.x, g.z);
                         const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), g.x, g.z);
@@ -371,9 +382,11 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
                         const unsigned a = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
                         const unsigned f = seg_full(a, g.y, g.z, thr, py0, m0, m1);
                         adm = a != 0u;
+                        done = done || f == 3u;
                         m0 = (f & 1u) ? kSegAlways : (a & 1u) ? m0 : kSegNever;
                         m1 = (f & 2u) ? kSegAlways : (a & 2u) ? m1 : kSegNever;
                     }
+                    if (done) list[first + off + tid] = id | kListDone;
                     const unsigned bal = __ballot_sync(0xffffffffu, adm);
                     uint32_t base = 0;
                     if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
@@ -404,7 +417,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, const uint32_t 
 
 }  // namespace
 
-int launch_raster_additive_mma(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
+int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const uint64_t *bin_offset,
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
                                WorkHead *head, cudaStream_t st)
 {
