@@ -58,8 +58,11 @@ struct SmemMma {
     union {
         struct {
             float B[2][2][2][kMmaBatch * kBlockPx];          // [buf][g][hi | lo][((p / 4) * 64 + j) * 4 + p % 4]
-            float4 qA[3][kQueue];                            // per channel: sx, c, a_channel, -
-            float4 qB[kQueue];                               // sy, c, segment minimum of group 0, of group 1 (folded)
+            // queue of admitted splats, stored by PAIRS (2 q, 2 q + 1) for the packed f32x2 arithmetic
+            float4 qG[kQueue / 2];                           // -sx0, -sx1, c0, c1
+            float2 qAmp[3][kQueue / 2];                      // per channel: a0, a1
+            float4 qBg[kQueue / 2];                          // -sy0, -sy1, c0, c1
+            float4 qBm[kQueue / 2];                          // folded segment minima: group 0 (splat 0, 1), group 1 (splat 0, 1)
         } w;
         float stage[kBlockPx][kBlockPx * 3];                 // flush only
     };
@@ -129,6 +132,31 @@ __device__ __forceinline__ void split_tf32(float v, uint32_t &hi, uint32_t &lo)
     lo = __float_as_uint(__fsub_rn(v, __uint_as_float(hi)));
 }
 
+__device__ __forceinline__ void queue_put(SmemMma &sm, uint32_t s, float sx, float sy, float c, float ar, float ag, float ab,
+                                          float m0, float m1)
+{
+    const uint32_t q = s >> 1, h = s & 1u;
+    float *G = reinterpret_cast<float *>(&sm.w.qG[q]), *Bg = reinterpret_cast<float *>(&sm.w.qBg[q]);
+    float *Bm = reinterpret_cast<float *>(&sm.w.qBm[q]);
+    G[h] = -sx;  G[2 + h] = c;
+    Bg[h] = -sy; Bg[2 + h] = c;
+    Bm[h] = m0;  Bm[2 + h] = m1;
+    reinterpret_cast<float *>(&sm.w.qAmp[0][q])[h] = ar;
+    reinterpret_cast<float *>(&sm.w.qAmp[1][q])[h] = ag;
+    reinterpret_cast<float *>(&sm.w.qAmp[2][q])[h] = ab;
+}
+
+// v = hi + lo for both halves of a packed pair (Veltkamp split with 2^13 + 1: hi has 11 significant bits,
+// i.e. it is a TF32 number; lo = v - hi is exact; the tensor core ignores the 13 low bits of lo)
+__device__ __forceinline__ void split_tf32x2(float2 v, float2 &hi, float2 &lo)
+{
+    const float2 m1 = make_float2(-1.0f, -1.0f);
+    const float2 gm = __fmul2_rn(v, make_float2(8193.0f, 8193.0f));
+    const float2 d = __ffma2_rn(v, m1, gm);          // gm - v
+    hi = __ffma2_rn(d, m1, gm);                      // gm - (gm - v)
+    lo = __ffma2_rn(hi, m1, v);                      // v - hi
+}
+
 __global__ void __launch_bounds__(kMmaThreads, 2)
 raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__restrict__ list,
                            const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
@@ -177,6 +205,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     bool fresh = true;                                    // D holds nothing yet: the first MMAs overwrite it
     int px0 = 0, py0 = 0;
 
+    constexpr uint32_t kBBytes = kMmaBatch * kBlockPx * 4;             // one B operand (16 splats x 64 rows)
+    constexpr uint64_t kStepUnits = (8 * kBlockPx * 4) >> 4;           // 16-byte units per K step (two K chunks)
+    const uint64_t bdesc0 = b_descriptor(&sm.w.B[0][0][0][0]);
+
     // ---- nb batches of 16 queued splats; every role walks the same sequence ----
     auto process_batches = [&](uint32_t nb) {
         for (uint32_t it = 0; it < nb; ++it) {
@@ -189,15 +221,15 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
 #pragma unroll
                     for (int g = 0; g < 2; ++g) {
                         const uint32_t d = tmem + kDCol + g * 64;
-                        const uint64_t b_hi = b_descriptor(sm.w.B[buf][g][0]), b_lo = b_descriptor(sm.w.B[buf][g][1]);
-#pragma unroll
-                        for (int s = 0; s < 2; ++s) {
-                            const uint32_t a_hi = tmem + kACol + buf * 64 + g * 32 + 8 * s, a_lo = a_hi + 16;
-                            const uint64_t step = (uint64_t)((8 * kBlockPx * 4) >> 4) * s;      // two 16-byte K chunks per step
-                            mma_tf32_ts(d, a_hi, b_hi + step, kIdesc, (fresh && s == 0) ? 0u : 1u);
-                            mma_tf32_ts(d, a_lo, b_hi + step, kIdesc, 1u);
-                            mma_tf32_ts(d, a_hi, b_lo + step, kIdesc, 1u);
-                        }
+                        const uint32_t a0 = tmem + kACol + buf * 64 + g * 32;
+                        const uint64_t b_hi = bdesc0 + (uint64_t)(((buf * 2 + g) * 2 + 0) * kBBytes >> 4);
+                        const uint64_t b_lo = bdesc0 + (uint64_t)(((buf * 2 + g) * 2 + 1) * kBBytes >> 4);
+                        mma_tf32_ts(d, a0, b_hi, kIdesc, fresh ? 0u : 1u);                 // K step 0: splats 0..7
+                        mma_tf32_ts(d, a0 + 16, b_hi, kIdesc, 1u);
+                        mma_tf32_ts(d, a0, b_lo, kIdesc, 1u);
+                        mma_tf32_ts(d, a0 + 8, b_hi + kStepUnits, kIdesc, 1u);             // K step 1: splats 8..15
+                        mma_tf32_ts(d, a0 + 24, b_hi + kStepUnits, kIdesc, 1u);
+                        mma_tf32_ts(d, a0 + 8, b_lo + kStepUnits, kIdesc, 1u);
                     }
                     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
                                  ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
@@ -208,12 +240,21 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                 if (a_warp) {
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const float x = pixel_centre(px0 + kSegPx * grp + lane);
-                    const float4 *qa = &sm.w.qA[quarter][q_head & (kQueue - 1)];   // a batch never wraps: 16 | kQueue
+                    const float2 xx = make_float2(x, x);
+                    const uint32_t qp = (q_head & (kQueue - 1)) >> 1;              // a batch never wraps: 16 | kQueue
+                    const float4 *qg = &sm.w.qG[qp];
+                    const float2 *qa = &sm.w.qAmp[quarter][qp];
                     uint32_t hi[16], lo[16];
 #pragma unroll
-                    for (int k = 0; k < kMmaBatch; ++k) {
-                        const float4 q = qa[k];
-                        split_tf32(__fmul_rn(q.z, gauss1d(x, q.x, q.y)), hi[k], lo[k]);
+                    for (int k = 0; k < kMmaBatch / 2; ++k) {                      // two splats per step, f32x2 arithmetic
+                        const float4 q = qg[k];
+                        float2 t = __fmul2_rn(__fadd2_rn(xx, make_float2(q.x, q.y)), make_float2(q.z, q.w));
+                        t = __fmul2_rn(t, t);
+                        const float2 v = __fmul2_rn(qa[k], make_float2(ex2_approx(-t.x), ex2_approx(-t.y)));
+                        float2 h, l;
+                        split_tf32x2(v, h, l);
+                        hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
+                        lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
                     }
                     const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
                     tmem_st16(a, hi);
@@ -223,26 +264,33 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                 } else {
                     const int j = b_rows * 32 + lane;
                     const float y = pixel_centre(py0 + j);
-                    const float4 *qb = &sm.w.qB[q_head & (kQueue - 1)];
+                    const float2 yy = make_float2(y, y);
+                    const uint32_t qp = (q_head & (kQueue - 1)) >> 1;
+                    const float4 *qg = &sm.w.qBg[qp], *qm = &sm.w.qBm[qp];
 #pragma unroll
                     for (int qq = 0; qq < 2; ++qq) {
-                        const int q4 = 2 * b_half + qq;                           // group of 4 splats
-                        uint32_t bh[2][4], bl[2][4];
+                        const int q4 = 2 * b_half + qq;                           // group of 4 splats = 2 pairs
+                        float2 bh[2][2], bl[2][2];                                // [group][pair]
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            const float4 q = qb[4 * q4 + k];
-                            const float gy = gauss1d(y, q.x, q.y);
-                            uint32_t ghi, glo;
-                            split_tf32(gy, ghi, glo);
-                            const bool h0 = seg_covered(q.z, gy, thr), h1 = seg_covered(q.w, gy, thr);
-                            bh[0][k] = h0 ? ghi : 0u;  bl[0][k] = h0 ? glo : 0u;
-                            bh[1][k] = h1 ? ghi : 0u;  bl[1][k] = h1 ? glo : 0u;
+                        for (int k = 0; k < 2; ++k) {
+                            const float4 q = qg[2 * q4 + k], m = qm[2 * q4 + k];
+                            // same operations, same roundings as gauss1d / seg_covered (raster_common.cuh), two splats at a time
+                            float2 t = __fmul2_rn(__fadd2_rn(yy, make_float2(q.x, q.y)), make_float2(q.z, q.w));
+                            t = __fmul2_rn(t, t);
+                            const float2 gy = make_float2(ex2_approx(-t.x), ex2_approx(-t.y));
+                            const float2 c0 = __fmul2_rn(make_float2(m.x, m.y), gy), c1 = __fmul2_rn(make_float2(m.z, m.w), gy);
+                            const float2 f0 = make_float2(c0.x >= thr ? 1.0f : 0.0f, c0.y >= thr ? 1.0f : 0.0f);
+                            const float2 f1 = make_float2(c1.x >= thr ? 1.0f : 0.0f, c1.y >= thr ? 1.0f : 0.0f);
+                            float2 h, l;
+                            split_tf32x2(gy, h, l);
+                            bh[0][k] = __fmul2_rn(h, f0);  bl[0][k] = __fmul2_rn(l, f0);
+                            bh[1][k] = __fmul2_rn(h, f1);  bl[1][k] = __fmul2_rn(l, f1);
                         }
                         const int at = (q4 * kBlockPx + j) * 4;
 #pragma unroll
                         for (int g = 0; g < 2; ++g) {
-                            *reinterpret_cast<uint4 *>(&sm.w.B[buf][g][0][at]) = make_uint4(bh[g][0], bh[g][1], bh[g][2], bh[g][3]);
-                            *reinterpret_cast<uint4 *>(&sm.w.B[buf][g][1][at]) = make_uint4(bl[g][0], bl[g][1], bl[g][2], bl[g][3]);
+                            *reinterpret_cast<float4 *>(&sm.w.B[buf][g][0][at]) = make_float4(bh[g][0].x, bh[g][0].y, bh[g][1].x, bh[g][1].y);
+                            *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0].x, bl[g][0].y, bl[g][1].x, bl[g][1].y);
                         }
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -266,8 +314,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         const uint32_t pad = kMmaBatch - rem;
         if ((uint32_t)tid < pad) {
             const uint32_t s = (tail + tid) & (kQueue - 1);
-            sm.w.qA[0][s] = sm.w.qA[1][s] = sm.w.qA[2][s] = make_float4(0.f, 0.f, 0.f, 0.f);
-            sm.w.qB[s] = make_float4(0.f, 0.f, kSegNever, kSegNever);
+            queue_put(sm, s, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, kSegNever, kSegNever);
         }
         if (tid == 0) sm.q_tail = tail + pad;
         __syncthreads();
@@ -394,10 +441,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                     if (adm) {
                         const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
                         const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
-                        sm.w.qA[0][s] = make_float4(g.x, g.z, amp.x, 0.f);
-                        sm.w.qA[1][s] = make_float4(g.x, g.z, amp.y, 0.f);
-                        sm.w.qA[2][s] = make_float4(g.x, g.z, amp.z, 0.f);
-                        sm.w.qB[s] = make_float4(g.y, g.z, m0, m1);
+                        queue_put(sm, s, g.x, g.y, g.z, amp.x, amp.y, amp.z, m0, m1);
                     }
                 }
                 __syncthreads();
