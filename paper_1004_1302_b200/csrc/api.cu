@@ -103,6 +103,7 @@ int make_render_const(const splotch_camera *cam, const splotch_colormap *cm, con
     o->support_f = p->support_f;
     o->z_near = p->z_near;
     o->thr = (float)exp(-(double)p->support_f * (double)p->support_f);
+    if (!(o->thr >= 1.17549435e-38f)) o->thr = 1.17549435e-38f;   // beyond f ~ 9.3 fp32 weights underflow anyway; keeps thr / gy > 0
     o->n_entries = cm ? cm->n_entries : 2;
     o->n_types = cm ? cm->n_types : 1;
     o->mode = p->mode;

@@ -40,9 +40,13 @@ struct SmemAdd {
 };
 
 // one (splat, tile) pair: this lane's 8 pixels of row `y` of the tile, channels packed as f32x2
-// The row record's fourth word is the coverage threshold thr / gy with two flags folded in: its
-// sign bit says "segment 0 of this row is handled by the tensor-core kernel", its lowest mantissa
-// bit the same for segment 1 (raster_common.cuh: seg_handled); a handled segment contributes 0 here.
+// The row record's fourth word is W = T' * 2^60, T' the float just below the coverage threshold
+// T = thr / gy, so that  sat(gx * 2^60 - W)  is exactly the indicator [gx >= T] (the difference of two
+// distinct floats of this range times 2^60 is >= 1): the mask costs one FFMA.SAT per pixel on the
+// FMA pipe instead of a compare and a select.  Two flags are folded into W: its sign bit says
+// "segment 0 of this row is handled by the tensor-core kernel", its lowest mantissa bit the same for
+// segment 1 (raster_common.cuh: seg_handled); a handled segment contributes 0 here.
+constexpr float kMaskScale = 1152921504606846976.0f;   // 2^60
 template <bool kRim>
 __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const float4 *__restrict__ rows, int x, int y,
                                            float2 (&acc)[3][4])
@@ -54,11 +58,12 @@ __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const 
     if (kRim) {
         const uint32_t wb = __float_as_uint(r.w);
         const bool handled = (x & kSegPx) ? (wb & 1u) != 0u : (wb >> 31) != 0u;
-        const float T = handled ? __int_as_float(0x7f800000) : fabsf(r.w);
+        const float nW = handled ? __int_as_float(0xff800000) : -fabsf(r.w);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            p[q].x = p[q].x >= T ? p[q].x : 0.0f;
-            p[q].y = p[q].y >= T ? p[q].y : 0.0f;
+            const float2 f = make_float2(__saturatef(__fmaf_rn(p[q].x, kMaskScale, nW)),
+                                         __saturatef(__fmaf_rn(p[q].y, kMaskScale, nW)));
+            p[q] = __fmul2_rn(p[q], f);
         }
     }
     const float2 wr = make_float2(r.x, r.x), wg = make_float2(r.y, r.y), wb = make_float2(r.z, r.z);
@@ -142,14 +147,18 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                 g = *reinterpret_cast<const float4 *>(&sm.rec[slot][s]);        // sx, sy, c, R
                 a = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 1);  // a_r, a_g, a_b, bins
             }
+            // packed f32x2 arithmetic throughout; every value that enters the split predicate is produced by the
+            // same correctly rounded operations as gauss1d / seg_covered (raster_common.cuh)
+            const float2 cc = make_float2(g.z, g.z), nsx = make_float2(-g.x, -g.x), nsy = make_float2(-g.y, -g.y);
             float4 v[2];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {           // columns part*4 + 32h .. +3: conflict-free 128-bit stores
-                const int c0 = px0 + part * 4 + 32 * h;
-                v[h].x = gauss1d(pixel_centre(c0), g.x, g.z);
-                v[h].y = gauss1d(pixel_centre(c0 + 1), g.x, g.z);
-                v[h].z = gauss1d(pixel_centre(c0 + 2), g.x, g.z);
-                v[h].w = gauss1d(pixel_centre(c0 + 3), g.x, g.z);
+                const float xb = pixel_centre(px0 + part * 4 + 32 * h);
+                float2 t0 = __fmul2_rn(__fadd2_rn(__fadd2_rn(make_float2(xb, xb), make_float2(0.0f, 1.0f)), nsx), cc);
+                float2 t1 = __fmul2_rn(__fadd2_rn(__fadd2_rn(make_float2(xb, xb), make_float2(2.0f, 3.0f)), nsx), cc);
+                t0 = __fmul2_rn(t0, t0);
+                t1 = __fmul2_rn(t1, t1);
+                v[h] = make_float4(ex2_approx(-t0.x), ex2_approx(-t0.y), ex2_approx(-t1.x), ex2_approx(-t1.y));
                 *reinterpret_cast<float4 *>(&sm.gx[slot][s][part * 4 + 32 * h]) = v[h];
             }
             // segments handled by the tensor-core kernel (same predicate, same bits: raster_common.cuh)
@@ -165,16 +174,30 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                 }
             }
             unsigned hb0 = 0u, hb1 = 0u;            // bit k: row part + 8k handled in segment 0 / 1
+            const float yb = pixel_centre(py0 + part);
+            const float2 thr2 = make_float2(thr, thr), scale2 = make_float2(kMaskScale, kMaskScale);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {           // rows part + 8k
-                const int j = part + 8 * k;
-                const float gy = gauss1d(pixel_centre(py0 + j), g.y, g.z);
-                const float T = row_threshold(thr, gy);
-                const unsigned hd = seg_handled(adm, full, m0, m1, gy, thr);
-                hb0 |= (hd & 1u) << k;
-                hb1 |= (hd >> 1) << k;
-                const uint32_t w = (__float_as_uint(T) & 0x7ffffffeu) | ((hd & 1u) << 31) | (hd >> 1);
-                sm.row[slot][s][j] = make_float4(a.x * gy, a.y * gy, a.z * gy, __uint_as_float(w));
+            for (int k = 0; k < 8; k += 2) {        // rows part + 8k, part + 8(k+1)
+                float2 t = __fmul2_rn(__fadd2_rn(__fadd2_rn(make_float2(yb, yb), make_float2(8.0f * k, 8.0f * k + 8.0f)), nsy), cc);
+                t = __fmul2_rn(t, t);
+                const float2 gy = make_float2(ex2_approx(-t.x), ex2_approx(-t.y));
+                float2 T = __fmul2_rn(thr2, make_float2(rcp_approx(gy.x), rcp_approx(gy.y)));      // used by this kernel only
+                T = make_float2(__uint_as_float(__float_as_uint(T.x) - 1u), __uint_as_float(__float_as_uint(T.y) - 1u));
+                const float2 Wm = __fmul2_rn(T, scale2);
+                unsigned hd0 = 0u, hd1 = 0u;        // handled bits (segment 0 | segment 1 << 1) of the two rows
+                if (adm) {
+                    const float2 c0 = __fmul2_rn(make_float2(m0, m0), gy), c1 = __fmul2_rn(make_float2(m1, m1), gy);
+                    hd0 = adm & (full | (c0.x >= thr ? 1u : 0u) | (c1.x >= thr ? 2u : 0u));
+                    hd1 = adm & (full | (c0.y >= thr ? 1u : 0u) | (c1.y >= thr ? 2u : 0u));
+                }
+                hb0 |= ((hd0 & 1u) << k) | ((hd1 & 1u) << (k + 1));
+                hb1 |= ((hd0 >> 1) << k) | ((hd1 >> 1) << (k + 1));
+                const uint32_t w0 = (__float_as_uint(Wm.x) & 0x7ffffffeu) | ((hd0 & 1u) << 31) | (hd0 >> 1);
+                const uint32_t w1 = (__float_as_uint(Wm.y) & 0x7ffffffeu) | ((hd1 & 1u) << 31) | (hd1 >> 1);
+                const float2 wr = __fmul2_rn(make_float2(a.x, a.x), gy), wg = __fmul2_rn(make_float2(a.y, a.y), gy);
+                const float2 wb = __fmul2_rn(make_float2(a.z, a.z), gy);
+                sm.row[slot][s][part + 8 * k] = make_float4(wr.x, wg.x, wb.x, __uint_as_float(w0));
+                sm.row[slot][s][part + 8 * k + 8] = make_float4(wr.y, wg.y, wb.y, __uint_as_float(w1));
             }
             unsigned all0 = hb0, all1 = hb1, any0 = hb0, any1 = hb1;
             if (mma_on) {

@@ -16,6 +16,13 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
