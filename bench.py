@@ -166,6 +166,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--force-tensor", action="store_true", help="additive mode: SPLOTCH_FORCE_TENSOR")
     ap.add_argument("--no-tensor", action="store_true", help="additive mode: SPLOTCH_NO_TENSOR (everything on the FP32 ALUs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -196,7 +197,7 @@ def main():
         raise SystemExit("multi-GPU sharding is defined for the additive mode only (DESIGN.md 'Multi-GPU')")
     cam = w.camera
     sc = Scene(w, dev)
-    sc.tensor = not args.no_tensor
+    sc.tensor = False if args.no_tensor else True if args.force_tensor else None
     vis, pairs, updates = sc.stats()
     sc.reserve(max_pairs=pairs + 1024)
     log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g}, "

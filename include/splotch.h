@@ -89,8 +89,11 @@ typedef struct {
 typedef enum { SPLOTCH_ADDITIVE = 0, SPLOTCH_ABSORB = 1 } splotch_mode;
 
 #define SPLOTCH_RAW_SUM 1u /* additive mode writes S_c = sum_p E_pc tau_p, not 1 - exp(-S_c)   */
-#define SPLOTCH_NO_TENSOR 2u /* additive mode: accumulate every pixel on the FP32 ALUs; by default the
-                              fully covered row segments of big splats run as split-TF32 tcgen05 MMAs */
+#define SPLOTCH_NO_TENSOR 2u /* additive mode: accumulate every pixel on the FP32 ALUs */
+#define SPLOTCH_FORCE_TENSOR 4u /* additive mode: always run the fully covered 32-pixel row segments of big
+                              splats as split-TF32 tcgen05 MMAs.  With neither flag the library decides on the
+                              device (no host sync): tensor cores when >= 75 % of the estimated pixel updates
+                              lie in such segments.  The image is the same within rounding either way. */
 
 typedef struct {
     float brightness[SPLOTCH_MAX_TYPES];     /* scales E per type                             */
@@ -98,7 +101,7 @@ typedef struct {
     int32_t mode;                            /* splotch_mode                                  */
     float support_f;                         /* f of PAPER.md:69; > 0; the configs use 3      */
     float z_near;                            /* cull view-space depth <= z_near               */
-    uint32_t flags;                          /* SPLOTCH_RAW_SUM | SPLOTCH_NO_TENSOR           */
+    uint32_t flags;                          /* SPLOTCH_RAW_SUM | NO_TENSOR | FORCE_TENSOR     */
 } splotch_params;
 
 /* ------------------------------------------------------------------------------------------

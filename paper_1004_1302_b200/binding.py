@@ -26,6 +26,7 @@ SPLOTCH_ADDITIVE = 0
 SPLOTCH_ABSORB = 1
 SPLOTCH_RAW_SUM = 1
 SPLOTCH_NO_TENSOR = 2
+SPLOTCH_FORCE_TENSOR = 4
 
 # every symbol include/splotch.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [

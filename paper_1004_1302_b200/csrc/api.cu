@@ -368,10 +368,10 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
     prof_mark(3, c.st);
     if (absorb) prof_mark(4, c.st);
     if (!absorb) {
-        const int mma_on = (params->flags & SPLOTCH_NO_TENSOR) ? 0 : 1;
+        const int mma_on = (params->flags & SPLOTCH_NO_TENSOR) ? 0 : (params->flags & SPLOTCH_FORCE_TENSOR) ? 1 : 2;
         if (mma_on) {
             rc = launch_raster_additive_mma(c.at<SplatAdd>(c.L.records), list, c.at<uint64_t>(c.L.bin_offset),
-                                            c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), c.st);
+                                            c.at<uint32_t>(c.L.unit_prefix), c.rc, c.cam, out_rgb, c.head(), mma_on, c.st);
             if (rc) return rc;
         }
         prof_mark(4, c.st);

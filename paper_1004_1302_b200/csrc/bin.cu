@@ -87,6 +87,7 @@ finish_offsets_kernel(const uint32_t *__restrict__ bin_count, const uint64_t *__
         head->n_units = 0;
         head->work_counter = 0;
         head->mma_counter = 0;
+        head->tensor_on = head->area_tensor >= kTensorShare * head->area_total && head->area_total > 0.0f ? 1u : 0u;
         if (D > max_pairs) head->status = -2;   // SPLOTCH_ERR_WORKSPACE
     }
     __syncthreads();

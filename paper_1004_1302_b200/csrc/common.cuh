@@ -82,7 +82,10 @@ struct WorkHead {
     uint32_t work_counter;          // persistent-kernel ticket
     uint32_t scan_ticket;           // decoupled look-back tile ticket
     uint32_t mma_counter;           // ticket of the tensor-core rasteriser
-    uint32_t pad[5];
+    float area_total;               // K1: sum of pi/4 x pixel-box areas of the visible splats (~ pixel updates)
+    float area_tensor;              // K1: estimate of the part of it inside fully covered 32-pixel row segments
+    uint32_t tensor_on;             // finish_offsets: area_tensor >= kTensorShare * area_total
+    uint32_t pad[2];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -158,14 +161,17 @@ int launch_iota(uint32_t *v, int64_t n, cudaStream_t st);
 
 // raster.cu (K3, K4)
 constexpr uint32_t kChunkAdd = 2048;   // splats per additive work unit
+// Additive mode: the tensor-core kernel pays off when most pixel updates lie in fully covered row segments
+// (measured: C3, share 0.83, step 476 -> 402 ms; C2, share 0.65, step 37 -> 45 ms).  tensor: 0 off, 1 on, 2 auto.
+constexpr float kTensorShare = 0.75f;
 constexpr uint32_t kChunkAbs = 4096;   // splats per absorb work unit
 int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                           WorkHead *head, int mma_on, cudaStream_t st);
+                           WorkHead *head, int tensor, cudaStream_t st);
 // raster_mma.cu: the fully covered row segments of the additive mode on the tensor cores
 int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const uint64_t *bin_offset,
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                               WorkHead *head, cudaStream_t st);
+                               WorkHead *head, int tensor, cudaStream_t st);
 int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const uint64_t *bin_offset,
                          const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam,
                          float *partials, WorkHead *head, cudaStream_t st);

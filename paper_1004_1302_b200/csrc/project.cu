@@ -114,14 +114,16 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
 {
     extern __shared__ uint32_t s_hist[];
     __shared__ unsigned int s_visible;
+    __shared__ float s_area[2];
     const int n_bins = rc.nbx * rc.nby;
     if (smem_hist)
         for (int i = threadIdx.x; i < n_bins; i += blockDim.x) s_hist[i] = 0u;
-    if (threadIdx.x == 0) s_visible = 0u;
+    if (threadIdx.x == 0) { s_visible = 0u; s_area[0] = s_area[1] = 0.0f; }
     __syncthreads();
     uint32_t *hist = smem_hist ? s_hist : bin_count;
 
     unsigned int my_visible = 0;
+    float my_area = 0.0f, my_tensor = 0.0f;     // heuristic for WorkHead::tensor_on, not part of the result
     const long long groups = (n + 3) / 4;
     const long long stride = (long long)gridDim.x * blockDim.x;
     // warp-uniform trip count: every lane of a warp runs the same number of iterations
@@ -174,6 +176,11 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
             const uint32_t bins = o.visible ? pack_bins(o, rc.bin_shift) : kInvisible;
             if (in) {
                 my_visible += o.visible ? 1u : 0u;
+                if (o.visible) {
+                    const float area = 0.78539816f * (float)(o.i1 - o.i0 + 1) * (float)(o.j1 - o.j0 + 1);
+                    my_area += area;
+                    if (o.R >= 15.5f) my_tensor += fmaxf(area - 64.0f * o.R, 0.0f);   // minus a 16-pixel band on both edges of every row
+                }
                 const float tau0 = (Iv[k] * rv[k]) * kSqrtPi;
                 const float cw = o.visible ? kSqrtLog2e / o.ss : 0.0f;
                 float er = 0.f, eg = 0.f, eb = 0.f;
@@ -207,6 +214,11 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
         }
     }
     atomicAdd(&s_visible, my_visible);
+    for (int d = 16; d > 0; d >>= 1) {
+        my_area += __shfl_xor_sync(0xffffffffu, my_area, d);
+        my_tensor += __shfl_xor_sync(0xffffffffu, my_tensor, d);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_area[0], my_area); atomicAdd(&s_area[1], my_tensor); }
     __syncthreads();
     if (smem_hist && bin_count) {
         for (int i = threadIdx.x; i < n_bins; i += blockDim.x) {
@@ -214,7 +226,11 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
             if (c) atomicAdd(&bin_count[i], c);
         }
     }
-    if (threadIdx.x == 0 && s_visible) atomicAdd(&head->visible, (unsigned long long)s_visible);
+    if (threadIdx.x == 0 && s_visible) {
+        atomicAdd(&head->visible, (unsigned long long)s_visible);
+        atomicAdd(&head->area_total, s_area[0]);
+        atomicAdd(&head->area_tensor, s_area[1]);
+    }
 }
 
 }  // namespace

@@ -78,8 +78,9 @@ __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const 
 __global__ void __launch_bounds__(kRasThreads, 2)
 raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
                        const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
-                       int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok, int mma_on)
+                       int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok, int tensor)
 {
+    const int mma_on = tensor == 2 ? (int)head->tensor_on : tensor;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SmemAdd &sm = *reinterpret_cast<SmemAdd *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -308,7 +309,7 @@ normalize_kernel(const float *__restrict__ S, float *__restrict__ out, long long
 
 int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const uint64_t *bin_offset,
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                           WorkHead *head, int mma_on, cudaStream_t st)
+                           WorkHead *head, int tensor, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
@@ -318,7 +319,7 @@ int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const 
     }
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
     raster_additive_kernel<<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(
-        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, mma_on);
+        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);
     SPLOTCH_LAUNCH_CHECK();
     return 0;
 }

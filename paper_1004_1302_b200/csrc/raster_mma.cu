@@ -160,8 +160,9 @@ __device__ __forceinline__ void split_tf32x2(float2 v, float2 &hi, float2 &lo)
 __global__ void __launch_bounds__(kMmaThreads, 2)
 raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__restrict__ list,
                            const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
-                           int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok)
+                           int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok, int tensor)
 {
+    if (tensor == 2 && head->tensor_on == 0u) return;     // auto: too little of the work is in full segments
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SmemMma &sm = *reinterpret_cast<SmemMma *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -463,7 +464,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
 
 int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const uint64_t *bin_offset,
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
-                               WorkHead *head, cudaStream_t st)
+                               WorkHead *head, int tensor, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
@@ -473,7 +474,7 @@ int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const ui
     }
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
     raster_additive_mma_kernel<<<sm_count() * 2, kMmaThreads, sizeof(SmemMma), st>>>(
-        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok);
+        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);
     SPLOTCH_LAUNCH_CHECK();
     return 0;
 }

@@ -39,7 +39,7 @@ class Scene:
         self.d = {}
         self.workspace: Optional[torch.Tensor] = None
         self.max_pairs = 0
-        self.tensor = True        # additive mode: fully covered row segments on the tensor cores (False: SPLOTCH_NO_TENSOR)
+        self.tensor = None        # additive mode: None = library decides, True = SPLOTCH_FORCE_TENSOR, False = SPLOTCH_NO_TENSOR
         if resident:
             self.upload()
 
@@ -62,7 +62,7 @@ class Scene:
 
     def params(self, mode: Optional[int] = None, raw: bool = False) -> B.splotch_params:
         w = self.w
-        flags = (B.SPLOTCH_RAW_SUM if raw else 0) | (0 if self.tensor else B.SPLOTCH_NO_TENSOR)
+        flags = (B.SPLOTCH_RAW_SUM if raw else 0) | (0 if self.tensor is None else B.SPLOTCH_FORCE_TENSOR if self.tensor else B.SPLOTCH_NO_TENSOR)
         return B.make_params(w.brightness, w.abs_brightness, w.mode if mode is None else mode, w.support_f, w.z_near, flags)
 
     def _alloc(self, nbytes: int) -> torch.Tensor:

@@ -26,9 +26,12 @@ def B():
     return binding
 
 
-def _scene(w):
+def _scene(w, tensor=None):
+    """tensor: None = the library decides, True = SPLOTCH_FORCE_TENSOR, False = SPLOTCH_NO_TENSOR."""
     from paper_1004_1302_b200 import Scene
-    return Scene(w)
+    sc = Scene(w)
+    sc.tensor = tensor
+    return sc
 
 
 def _tol_check(out, ref, what=""):
@@ -196,8 +199,8 @@ def test_bins_member_capacity_is_respected(B):
 # ------------------------------------------------------------------------------------------------
 # whole path: pixels
 # ------------------------------------------------------------------------------------------------
-def _render_both(w, raw=False, mode=None):
-    sc = _scene(w)
+def _render_both(w, raw=False, mode=None, tensor=None):
+    sc = _scene(w, tensor)
     out = sc.render(raw=raw, mode=mode)
     torch.cuda.synchronize()
     ref = oracle.render(w, raw=raw, mode=mode)
@@ -212,16 +215,41 @@ def test_additive_c1_full(B, raw):
     _tol_check(out, ref, "C1")
 
 
+@pytest.mark.parametrize("tensor", [None, True, False])
 @pytest.mark.parametrize("case", ["C2", "C3", "C5"])
-def test_additive_scaled_configs(B, case):
+def test_additive_scaled_configs(B, case, tensor):
     w = {"C2": lambda: workloads.make("C2", 200_000, width=512, height=512),
          "C3": lambda: workloads.make("C3", 300_000, width=600, height=360),        # ragged: not multiples of 64
          "C5": lambda: workloads.make("C5", 400_000, width=513, height=257)}[case]()  # odd width: scalar write path
-    out, ref = _render_both(w, raw=True)
+    out, ref = _render_both(w, raw=True, tensor=tensor)
     assert ref.mean() > 0.05
     _tol_check(out, ref, case)
-    out, ref = _render_both(w, raw=False)
+    out, ref = _render_both(w, raw=False, tensor=tensor)
     _tol_check(out, ref, case)
+
+
+@pytest.mark.parametrize("size", [(704, 512), (601, 333)])
+def test_tensor_path_big_bright_splats(B, size):
+    """Splats from 10 to 600 pixels wide with amplitudes up to ~0.3, centres on and off screen: most pixel
+    updates lie in fully covered 32-pixel row segments, i.e. on the tensor cores (split TF32, raster_mma.cu).
+    Checked against the oracle (rim pixels masked: a_c of order one, DESIGN.md error budget), against the
+    ALU-only path, and the automatic choice must reproduce one of the two."""
+    rs = np.random.RandomState(11)
+    n = 2500
+    c = cam(eye=(0.0, 0.0, -10.0), fov=25.0, w=size[0], h=size[1])
+    r = np.exp(rs.uniform(np.log(0.03), np.log(2.0), n))
+    pts = np.stack([rs.uniform(-3.5, 3.5, n), rs.uniform(-2.6, 2.6, n), rs.uniform(-1, 1, n), r,
+                    rs.uniform(0.02, 0.3, n) / r, rs.uniform(0, 1, n)], 1)
+    w = mk(pts, c, lut_e=workloads.lut_hot(), support_f=3.1)
+    ref = oracle.render(w, raw=True)
+    assert ref.max() > 20.0
+    outs = {}
+    for tensor in (True, False, None):
+        sc = _scene(w, tensor)
+        outs[tensor] = sc.render(raw=True).cpu().numpy()
+        _tol_check_masked(w, outs[tensor], ref, max_rim=0.10)
+    np.testing.assert_allclose(outs[True], outs[False], rtol=3e-5, atol=3e-5)
+    assert np.array_equal(outs[None], outs[True]) or np.allclose(outs[None], outs[False], rtol=1e-5, atol=1e-6)
 
 
 def test_absorb_scaled_c4(B):
@@ -258,7 +286,7 @@ def test_absorb_strong_absorption_and_zero_channel(B):
     _tol_check_masked(w, out, ref)
 
 
-def _tol_check_masked(w, out, ref):
+def _tol_check_masked(w, out, ref, max_rim=0.05):
     tab, ok = oracle.splat_table(w)
     H, W = ref.shape[:2]
     jj, ii = np.meshgrid(np.arange(H) + 0.5, np.arange(W) + 0.5, indexing="ij")
@@ -267,7 +295,7 @@ def _tol_check_masked(w, out, ref):
         d2 = (ii - tab[p, 0]) ** 2 + (jj - tab[p, 1]) ** 2
         rim |= np.abs(d2 - tab[p, 3] ** 2) < 1e-4 * tab[p, 3] ** 2
     err = np.abs(out - ref) / (1e-4 * np.maximum(1.0, np.abs(ref)))
-    assert rim.mean() < 0.05
+    assert rim.mean() < max_rim
     assert err[~rim].max() <= 1.0, err[~rim].max()
 
 
@@ -276,8 +304,9 @@ def test_single_splat_shapes(B):
     for r, f in [(0.0004, 3.1), (0.004, 3.1), (0.04, 3.1), (0.4, 3.1), (4.0, 3.1), (0.02, 5.0)]:
         c = cam(eye=(0.013, -0.007, -10.0), lookat=(0.013, -0.007, 0.0), fov=20.0, w=200, h=136)
         w = mk([(0.05, 0.02, 0.0, r, 1.0 / r, 0.3)], c, lut_e=const_lut((1.0, 0.6, 0.3)), support_f=f)
-        out, ref = _render_both(w, raw=True)
-        _tol_check_masked(w, out, ref)
+        for tensor in (True, False):
+            out, ref = _render_both(w, raw=True, tensor=tensor)
+            _tol_check_masked(w, out, ref)
         assert ref.max() > 0.05 or r < 0.001
 
 
@@ -313,7 +342,7 @@ def test_edge_cases(B):
 def test_repeat_calls_and_orbit_cameras(B):
     """C5's use case: several cameras over one resident particle set; same camera twice gives the same image."""
     w = workloads.make("C5", 300_000, width=256, height=256)
-    sc = _scene(w)
+    sc = _scene(w, tensor=True)
     worst_pairs = max(sc.count_pairs(cm)[0] for cm in w.cameras)
     sc.reserve(max_pairs=worst_pairs)
     first = None
