@@ -47,7 +47,10 @@ constexpr int kIssuerWarp = 10;
 constexpr int kMmaBatch = 16;             // splats per batch = two K = 8 steps
 constexpr int kQueue = 512;               // ring of admitted splats (power of two)
 constexpr int kFilterChunk = 256;         // list entries per filter pass (one per thread of warps 0-7)
-constexpr int kUnitsPerTicket = 8;
+// The tensor core adds every K = 8 dot product into the fp32 accumulator with truncation: a relative deficit of
+// ~2^-25 per MMA (measured on C3: -7e-5 with 8 units = ~3700 MMAs per accumulator between flushes).  Two units
+// (~900 MMAs) keep it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
+constexpr int kUnitsPerTicket = 2;
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
 constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
