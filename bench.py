@@ -44,10 +44,11 @@ def read_peaks():
     if os.path.exists(path):
         try:
             d = json.load(open(path))
-            return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+            return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)),
+                        bf16_tflops=float(d.get("bf16_tflops_sustained", d.get("bf16_tflops", 1379.5))), source="measured")
         except Exception:  # pragma: no cover
             pass
-    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, bf16_tflops=1379.5, source="fallback")
 
 
 def read_traffic(workload: str, kernel: str):
@@ -199,6 +200,7 @@ def main():
     sc = Scene(w, dev)
     sc.tensor = False if args.no_tensor else True if args.force_tensor else None
     vis, pairs, updates = sc.stats()
+    upd_tensor, tensor_on, tensor_share = sc.tensor_stats() if w.mode == 0 else (0, 0, 0.0)
     sc.reserve(max_pairs=pairs + 1024)
     log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g}, "
         f"workspace {sc.workspace.numel() / 2**30:.2f} GiB")
@@ -250,18 +252,39 @@ def main():
     total_particles = w.n * world
     value = total_particles / (ms_step * 1e-3) / 1e6
 
-    # ---- roofline of the dominant kernel (K3, the tile rasteriser): plain FP32 ALU bound ----
-    raster_ms = stage_ms[3] + stage_ms[4]
+    # ---- rooflines of the rasteriser (K3): plain FP32 ALU kernel, and in the additive mode the tensor-core kernel ----
+    tensor_ms, alu_ms = stage_ms[3], stage_ms[4]
+    raster_ms = tensor_ms + alu_ms
+    tensor_used = w.mode == 0 and tensor_ms > 0.05
     sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
     alu_peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12          # Tlane-op/s
     c_ops = ALGO_LANE_OPS_PER_UPDATE[w.mode]
-    alu_achieved = updates * c_ops / (raster_ms * 1e-3) / 1e12 if raster_ms > 0 else 0.0
-    traffic = read_traffic(w.name, "raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel")
-    roofline = dict(bound="alu", kernel="raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel",
-                    achieved=alu_achieved, peak=alu_peak, unit="Tlane-op/s", frac=alu_achieved / alu_peak if alu_peak else None,
-                    traffic=traffic, kernel_ms=raster_ms, kernel_share_of_step=raster_ms / ms_step if ms_step else None,
-                    updates_per_launch=updates, algorithmic_lane_ops_per_update=c_ops,
+    upd_alu = updates - (upd_tensor if tensor_used else 0)
+    alu_kernel = "raster_additive_kernel" if w.mode == 0 else "raster_absorb_kernel"
+    alu_achieved = upd_alu * c_ops / (alu_ms * 1e-3) / 1e12 if alu_ms > 0 else 0.0
+    alu_roof = dict(bound="alu", kernel=alu_kernel, achieved=alu_achieved, peak=alu_peak, unit="Tlane-op/s",
+                    frac=alu_achieved / alu_peak if alu_peak else None, traffic=read_traffic(w.name, alu_kernel),
+                    kernel_ms=alu_ms, kernel_share_of_step=alu_ms / ms_step if ms_step else None,
+                    updates_per_launch=upd_alu, algorithmic_lane_ops_per_update=c_ops,
                     peak_source=f"{sm_count} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} clock)")
+    tensor_roof = None
+    if tensor_used:
+        tf32_peak = 0.5 * peaks["bf16_tflops"]                                     # guide: TF32 dense = half of BF16
+        t_achieved = 2.0 * 3.0 * upd_tensor / (tensor_ms * 1e-3) / 1e12            # one multiply-add per channel per update
+        tensor_roof = dict(bound="tensor", kernel="raster_additive_mma_kernel", achieved=t_achieved, peak=tf32_peak,
+                           unit="TFLOP/s", frac=t_achieved / tf32_peak, traffic=read_traffic(w.name, "raster_additive_mma_kernel"),
+                           kernel_ms=tensor_ms, kernel_share_of_step=tensor_ms / ms_step, updates_per_launch=upd_tensor,
+                           algorithmic_flops_per_update=6.0,
+                           executed_over_algorithmic=4.0,   # 3 split-TF32 products x 128/96 padded accumulator rows
+                           peak_source=f"0.5 x sustained dense BF16 cuBLAS throughput ({peaks['source']}) = TF32 dense")
+    # the dominant kernel by time is the headline roofline; the whole rasteriser is also quoted in ALU terms
+    roofline = alu_roof if (not tensor_used or alu_ms >= tensor_ms) else tensor_roof
+    eq = updates * c_ops / (raster_ms * 1e-3) / 1e12 if raster_ms > 0 else 0.0
+    raster_equiv = dict(unit="Tlane-op/s", achieved=eq, peak=alu_peak, frac=eq / alu_peak if alu_peak else None,
+                        raster_ms=raster_ms, updates=updates, updates_on_tensor_cores=upd_tensor if tensor_used else 0,
+                        tensor_share_estimate=tensor_share, tensor_cores_used=bool(tensor_used),
+                        note="all K3 updates x algorithmic lane-ops / (tensor + ALU kernel time): what an ALU-only "
+                             "rasteriser would have to sustain to match")
     algo_bytes = w.n * w.bytes_per_particle + cam.width * cam.height * 12
     hbm_gbs = algo_bytes / (ms_step * 1e-3) / 1e9
     hbm = dict(algorithmic_bytes_per_step=algo_bytes, achieved_gbs=hbm_gbs, frac_of_measured=hbm_gbs / peaks["hbm_gbs"],
@@ -312,7 +335,8 @@ def main():
                                 seed=w.seed, visible=vis, pairs=pairs, pixel_updates=updates,
                                 pixels_per_s=cam.width * cam.height / (ms_step * 1e-3),
                                 updates_per_s=updates * world / (ms_step * 1e-3)),
-                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, hbm_roofline=hbm,
+                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline,
+                    roofline_alu=alu_roof, roofline_tensor=tensor_roof, raster_alu_equivalent=raster_equiv, hbm_roofline=hbm,
                     stage_ms=dict(zip(["project_count", "offsets", "lists", "raster_tensor", "raster_alu", "output_map"], stage_ms)),
                     cpu_baseline=cpu)
         print(json.dumps(line), flush=True)

@@ -198,6 +198,16 @@ int splotch_debug_stats(const splotch_particles *particles, int64_t n, const spl
                         uint64_t workspace_bytes, int32_t bin_shift, uint64_t *visible_host,
                         uint64_t *pairs_host, uint64_t *updates_host, void *stream);
 
+/* splotch_debug_tensor_stats (SYNCHRONISES; additive mode, production 64x64 bins; workspace as for
+ * splotch_debug_stats with bin_shift 6): host outputs: the number of pixel updates inside the image
+ * that the tensor-core rasteriser performs when it runs (32-pixel row segments for which its
+ * `handled` predicate holds), the library's own choice for this scene (1 = tensor cores), and the
+ * estimated share of updates in such segments on which that choice rests. */
+int splotch_debug_tensor_stats(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                               const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                               uint64_t workspace_bytes, uint64_t *updates_tensor_host, int32_t *tensor_on_host,
+                               float *share_host, void *stream);
+
 /* Device-wide building blocks, exported so that tests can check them in isolation.
  * splotch_debug_scan: out[k] = sum_{m<k} in[k] for k <= n (n+1 outputs, 64-bit), the
  *   single-pass decoupled look-back scan used for bin offsets.  scratch: >= (n/2048 + 2) * 8 + 256 bytes.

@@ -32,7 +32,7 @@ SPLOTCH_FORCE_TENSOR = 4
 EXPORTS = [
     "splotch_workspace_bytes", "splotch_render", "splotch_workspace_status", "splotch_count_pairs",
     "splotch_normalize", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
-    "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_scan",
+    "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_tensor_stats", "splotch_debug_scan",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
     "splotch_last_cuda_error", "splotch_version", "splotch_profile_enable", "splotch_profile_read",
     "splotch_launch_count",
@@ -254,6 +254,16 @@ def splotch_debug_stats(particles, n, camera, colormap, params, workspace, works
                                       C.c_int32(bin_shift), C.byref(vis), C.byref(pairs), C.byref(upd),
                                       _vp(_stream(stream))))
     return int(vis.value), int(pairs.value), int(upd.value)
+
+
+def splotch_debug_tensor_stats(particles, n, camera, colormap, params, workspace, workspace_bytes, stream=None):
+    """(updates on the tensor cores, tensor_on chosen by the library, estimated share); synchronises the stream."""
+    upd, on, share = C.c_uint64(0), C.c_int32(0), C.c_float(0.0)
+    _check("splotch_debug_tensor_stats",
+           _lib().splotch_debug_tensor_stats(C.byref(particles), C.c_int64(n), C.byref(camera), C.byref(colormap),
+                                             C.byref(params), _vp(_ptr(workspace)), C.c_uint64(workspace_bytes),
+                                             C.byref(upd), C.byref(on), C.byref(share), _vp(_stream(stream))))
+    return int(upd.value), int(on.value), float(share.value)
 
 
 def splotch_debug_scan(inp, out, n: int, scratch, scratch_bytes: int, stream=None) -> None:

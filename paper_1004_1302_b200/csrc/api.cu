@@ -596,6 +596,28 @@ int splotch_debug_stats(const splotch_particles *particles, int64_t n, const spl
     return SPLOTCH_OK;
 }
 
+int splotch_debug_tensor_stats(const splotch_particles *particles, int64_t n, const splotch_camera *camera,
+                               const splotch_colormap *colormap, const splotch_params *params, void *workspace,
+                               uint64_t workspace_bytes, uint64_t *updates_tensor_host, int32_t *tensor_on_host,
+                               float *share_host, void *stream)
+{
+    if (!params || params->mode != SPLOTCH_ADDITIVE) return SPLOTCH_ERR_INVALID_ARG;
+    Ctx c;
+    int rc = setup(particles, n, camera, colormap, params, kBlockShift, workspace, workspace_bytes, 0, false, stream, &c);
+    if (rc) return rc;
+    rc = run_front(c, particles, n, colormap, ~0ull, kChunkAdd, nullptr);
+    if (rc) return rc;
+    rc = launch_count_tensor_updates(c.at<SplatAdd>(c.L.records), n, c.rc, c.cam, c.head(), c.st);
+    if (rc) return rc;
+    WorkHead h;
+    SPLOTCH_CUDA_TRY(cudaMemcpyAsync(&h, c.ws + c.L.head, sizeof(h), cudaMemcpyDeviceToHost, c.st));
+    SPLOTCH_CUDA_TRY(cudaStreamSynchronize(c.st));
+    if (updates_tensor_host) *updates_tensor_host = h.updates_tensor;
+    if (tensor_on_host) *tensor_on_host = (int32_t)h.tensor_on;
+    if (share_host) *share_host = h.area_total > 0.0f ? h.area_tensor / h.area_total : 0.0f;
+    return SPLOTCH_OK;
+}
+
 int splotch_debug_scan(const uint32_t *in, uint64_t *out, int64_t n, void *scratch, uint64_t scratch_bytes, void *stream)
 {
     if (n < 0 || !out || (n > 0 && !in) || !scratch) return SPLOTCH_ERR_INVALID_ARG;

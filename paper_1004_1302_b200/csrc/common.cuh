@@ -85,7 +85,7 @@ struct WorkHead {
     float area_total;               // K1: sum of pi/4 x pixel-box areas of the visible splats (~ pixel updates)
     float area_tensor;              // K1: estimate of the part of it inside fully covered 32-pixel row segments
     uint32_t tensor_on;             // finish_offsets: area_tensor >= kTensorShare * area_total
-    uint32_t pad[2];
+    unsigned long long updates_tensor;   // debug_tensor_stats: updates the tensor-core kernel performs
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -177,6 +177,8 @@ int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const ui
                          float *partials, WorkHead *head, cudaStream_t st);
 int launch_merge_absorb(const float *partials, const uint32_t *unit_prefix, const RenderConst &rc,
                         const CameraConst &cam, float *out, const WorkHead *head, cudaStream_t st);
+int launch_count_tensor_updates(const SplatAdd *records, int64_t n, const RenderConst &rc, const CameraConst &cam,
+                                WorkHead *head, cudaStream_t st);
 int launch_normalize(const float *S, float *out, int64_t n_values, cudaStream_t st);
 
 }  // namespace splotch

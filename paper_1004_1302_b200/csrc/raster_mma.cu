@@ -463,7 +463,53 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
 }
 
+// Statistic for bench.py (not part of a render): the number of pixel updates inside the image that the
+// tensor-core kernel performs, i.e. 32 x (handled row segments), evaluated with the same predicates.
+// One warp per splat; lanes share the rows of every block of the splat's bin box.
+__global__ void __launch_bounds__(256)
+count_tensor_updates_kernel(const SplatAdd *__restrict__ records, long long n, int W, int H, float thr, WorkHead *head)
+{
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    unsigned long long total = 0;
+    for (long long i = warp0; i < n; i += n_warps) {
+        const float4 g = __ldg(reinterpret_cast<const float4 *>(records + i));
+        const uint32_t bins = __ldg(reinterpret_cast<const uint32_t *>(records + i) + 7);
+        if (bins == kInvisible || !(g.w >= 15.5f)) continue;
+        const int bx0 = bins & 255, bx1 = (bins >> 8) & 255, by0 = (bins >> 16) & 255, by1 = bins >> 24;
+        for (int by = by0; by <= by1; ++by)
+            for (int bx = bx0; bx <= bx1; ++bx) {
+                const int px0 = bx * kBlockPx, py0 = by * kBlockPx;
+                const float m0 = fminf(gauss1d(pixel_centre(px0), g.x, g.z), gauss1d(pixel_centre(px0 + kSegPx - 1), g.x, g.z));
+                const float m1 = fminf(gauss1d(pixel_centre(px0 + kSegPx), g.x, g.z),
+                                       gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), g.x, g.z));
+                const unsigned adm = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+                if (adm == 0u) continue;
+                const unsigned full = seg_full(adm, g.y, g.z, thr, py0, m0, m1);
+                const int w0 = min(max(W - px0, 0), kSegPx), w1 = min(max(W - px0 - kSegPx, 0), kSegPx);
+                for (int j = lane; j < kBlockPx; j += 32) {
+                    if (py0 + j >= H) continue;
+                    const unsigned hd = seg_handled(adm, full, m0, m1, gauss1d(pixel_centre(py0 + j), g.y, g.z), thr);
+                    total += (unsigned long long)(((hd & 1u) ? w0 : 0) + ((hd & 2u) ? w1 : 0));
+                }
+            }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
+    if (lane == 0 && total) atomicAdd(&head->updates_tensor, total);
+}
+
 }  // namespace
+
+int launch_count_tensor_updates(const SplatAdd *records, int64_t n, const RenderConst &rc, const CameraConst &cam,
+                                WorkHead *head, cudaStream_t st)
+{
+    if (n <= 0) return 0;
+    count_tensor_updates_kernel<<<sm_count() * 8, 256, 0, st>>>(records, (long long)n, cam.W, cam.H, rc.thr, head);
+    SPLOTCH_LAUNCH_CHECK();
+    return 0;
+}
 
 int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const uint64_t *bin_offset,
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,

@@ -122,6 +122,14 @@ class Scene:
         ws = self._alloc(nbytes)
         return B.splotch_debug_stats(self.particles(), self.n, cs, self.colormap(), ps, self._aligned(ws), nbytes, bin_shift)
 
+    def tensor_stats(self, cam=None):
+        """(updates the tensor-core rasteriser performs, the library's choice 0/1, estimated share); synchronises."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(0)
+        nbytes = B.splotch_debug_workspace_bytes(self.n, cs, ps, 6, 0)
+        ws = self._alloc(nbytes)
+        return B.splotch_debug_tensor_stats(self.particles(), self.n, cs, self.colormap(), ps, self._aligned(ws), nbytes)
+
     # ---- end to end with host buffers ---------------------------------------------------------
     def host_buffers(self, pinned: bool = True):
         """Pinned host copies of the inputs and a pinned output image for render_host."""
