@@ -248,10 +248,17 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
             while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
             m = __ballot_sync(0xffffffffu, cB == 2);
             while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
-            m = __ballot_sync(0xffffffffu, cA == 1);
-            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
-            m = __ballot_sync(0xffffffffu, cB == 1);
-            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
+            // rim tiles: the items of the two tiles are walked in pairs, two independent chains per iteration
+            unsigned mA = __ballot_sync(0xffffffffu, cA == 1), mB = __ballot_sync(0xffffffffu, cB == 1);
+            while (mA && mB) {
+                const int sA = __ffs(mA) - 1, sB = __ffs(mB) - 1;
+                mA &= mA - 1;
+                mB &= mB - 1;
+                splat_tile<true>(sm.gx[slot][sA], sm.row[slot][sA], xA, yA, accA);
+                splat_tile<true>(sm.gx[slot][sB], sm.row[slot][sB], xB, yB, accB);
+            }
+            while (mA) { const int s = __ffs(mA) - 1; mA &= mA - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
+            while (mB) { const int s = __ffs(mB) - 1; mB &= mB - 1; splat_tile<true>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
             cp_async_wait_all();
             __syncthreads();
         }
