@@ -160,7 +160,7 @@ int launch_expand_pairs(const void *records, int record_bytes, const uint32_t *s
 int launch_iota(uint32_t *v, int64_t n, cudaStream_t st);
 
 // raster.cu (K3, K4)
-constexpr uint32_t kChunkAdd = 2048;   // splats per additive work unit
+constexpr uint32_t kChunkAdd = 4096;   // splats per additive work unit
 // Additive mode: the tensor-core kernel pays off when most pixel updates lie in fully covered row segments
 // (measured: C3, share 0.83, step 476 -> 402 ms; C2, share 0.65, step 37 -> 45 ms).  tensor: 0 off, 1 on, 2 auto.
 constexpr float kTensorShare = 0.75f;

@@ -45,12 +45,14 @@ constexpr int kMmaThreads = 352;          // 11 warps
 constexpr int kProducerWarps = 10;
 constexpr int kIssuerWarp = 10;
 constexpr int kMmaBatch = 16;             // splats per batch = two K = 8 steps
-constexpr int kQueue = 512;               // ring of admitted splats (power of two)
-constexpr int kFilterChunk = 256;         // list entries per filter pass (one per thread of warps 0-7)
+constexpr int kFilterThreads = 256;       // warps 0-7 filter
+constexpr int kPerThread = 2;             // list entries per filter thread and pass
+constexpr int kFilterChunk = kFilterThreads * kPerThread;   // list entries per filter pass
+constexpr int kQueue = 1024;              // ring of admitted splats (power of two, > kFilterChunk + a batch)
 // The tensor core adds every K = 8 dot product into the fp32 accumulator with truncation: a relative deficit of
 // ~2^-25 per MMA (measured on C3: -7e-5 with 8 units = ~3700 MMAs per accumulator between flushes).  Two units
 // (~900 MMAs) keep it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
-constexpr int kUnitsPerTicket = 2;
+constexpr int kUnitsPerTicket = 1;
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
 constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
@@ -396,56 +398,66 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
             const unsigned long long first = sm.range[r].first;
             px0 = (bin % nbx) * kBlockPx;
             py0 = (bin / nbx) * kBlockPx;
-            // software-pipelined filter: ids two chunks ahead, records one chunk ahead
-            const bool filt = tid < kFilterChunk;
-            uint32_t id_cur = 0, id_next = 0;
-            float4 geo = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (filt) {
-                if ((uint32_t)tid < count) id_cur = list[first + tid];
-                if ((uint32_t)tid + kFilterChunk < count) id_next = list[first + kFilterChunk + tid];
-                if ((uint32_t)tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
+            // software-pipelined filter: ids two chunks ahead, records one chunk ahead; kPerThread entries per thread
+            const bool filt = tid < kFilterThreads;
+            uint32_t id_cur[kPerThread], id_next[kPerThread];
+            float4 geo[kPerThread];
+#pragma unroll
+            for (int e = 0; e < kPerThread; ++e) {
+                const uint32_t i = (uint32_t)(e * kFilterThreads + tid);
+                id_cur[e] = id_next[e] = 0u;
+                geo[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (filt) {
+                    if (i < count) id_cur[e] = list[first + i];
+                    if (i + kFilterChunk < count) id_next[e] = list[first + kFilterChunk + i];
+                    if (i < count) geo[e] = __ldg(reinterpret_cast<const float4 *>(records + id_cur[e]));
+                }
             }
             for (uint32_t off = 0; off < count; off += kFilterChunk) {
                 if (filt) {
-                    const float4 g = geo;
-                    const uint32_t id = id_cur;
-                    const bool have = off + tid < count;
-                    // prefetch for the next two chunks before the batches of this one
-                    id_cur = id_next;
-                    if (off + kFilterChunk + tid < count) geo = __ldg(reinterpret_cast<const float4 *>(records + id_cur));
-                    if (off + 2 * kFilterChunk + tid < count) id_next = list[first + off + 2 * kFilterChunk + tid];
-                    bool adm = false;
-                    float m0 = kSegNever, m1 = kSegNever;
-                    bool done = false;                     // nothing left for the ALU kernel in this block
-                    if (have) {                            // the circle misses the block (bins are pixel boxes: B-rules)
-                        const float x_lo = pixel_centre(px0), x_hi = pixel_centre(px0 + kBlockPx - 1);
-                        const float y_lo = pixel_centre(py0), y_hi = pixel_centre(py0 + kBlockPx - 1);
-                        const float nx = fmaxf(fmaxf(x_lo - g.x, g.x - x_hi), 0.0f), ny = fmaxf(fmaxf(y_lo - g.y, g.y - y_hi), 0.0f);
-                        done = __fmaf_rn(nx, nx, __fmul_rn(ny, ny)) > __fmul_rn(__fmul_rn(g.w, g.w), 1.00001f);
-                    }
-                    if (have && g.w >= 15.5f) {
-                        const float e0 = gauss1d(pixel_centre(px0), g.x, g.z);
-                        const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), g.x, g.z);
-                        const float e2 = gauss1d(pixel_centre(px0 + kSegPx), g.x, g.z);
-                        const float e3 = gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), g.x, g.z);
-                        m0 = fminf(e0, e1);
-                        m1 = fminf(e2, e3);
-                        const unsigned a = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
-                        const unsigned f = seg_full(a, g.y, g.z, thr, py0, m0, m1);
-                        adm = a != 0u;
-                        done = done || f == 3u;
-                        m0 = (f & 1u) ? kSegAlways : (a & 1u) ? m0 : kSegNever;
-                        m1 = (f & 2u) ? kSegAlways : (a & 2u) ? m1 : kSegNever;
-                    }
-                    if (done) list[first + off + tid] = id | kListDone;
-                    const unsigned bal = __ballot_sync(0xffffffffu, adm);
-                    uint32_t base = 0;
-                    if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
-                    base = __shfl_sync(0xffffffffu, base, 0);
-                    if (adm) {
-                        const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
-                        const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
-                        queue_put(sm, s, g.x, g.y, g.z, amp.x, amp.y, amp.z, m0, m1);
+#pragma unroll
+                    for (int e = 0; e < kPerThread; ++e) {
+                        const uint32_t i = off + (uint32_t)(e * kFilterThreads + tid);
+                        const float4 g = geo[e];
+                        const uint32_t id = id_cur[e];
+                        const bool have = i < count;
+                        // prefetch for the next two chunks before the batches of this one
+                        id_cur[e] = id_next[e];
+                        if (i + kFilterChunk < count) geo[e] = __ldg(reinterpret_cast<const float4 *>(records + id_cur[e]));
+                        if (i + 2 * kFilterChunk < count) id_next[e] = list[first + i + 2 * kFilterChunk];
+                        bool adm = false;
+                        float m0 = kSegNever, m1 = kSegNever;
+                        bool done = false;                     // nothing left for the ALU kernel in this block
+                        if (have) {                            // the circle misses the block (bins are pixel boxes: B-rules)
+                            const float x_lo = pixel_centre(px0), x_hi = pixel_centre(px0 + kBlockPx - 1);
+                            const float y_lo = pixel_centre(py0), y_hi = pixel_centre(py0 + kBlockPx - 1);
+                            const float nx = fmaxf(fmaxf(x_lo - g.x, g.x - x_hi), 0.0f), ny = fmaxf(fmaxf(y_lo - g.y, g.y - y_hi), 0.0f);
+                            done = __fmaf_rn(nx, nx, __fmul_rn(ny, ny)) > __fmul_rn(__fmul_rn(g.w, g.w), 1.00001f);
+                        }
+                        if (have && g.w >= 15.5f) {
+                            const float e0 = gauss1d(pixel_centre(px0), g.x, g.z);
+                            const float e1 = gauss1d(pixel_centre(px0 + kSegPx - 1), g.x, g.z);
+                            const float e2 = gauss1d(pixel_centre(px0 + kSegPx), g.x, g.z);
+                            const float e3 = gauss1d(pixel_centre(px0 + 2 * kSegPx - 1), g.x, g.z);
+                            m0 = fminf(e0, e1);
+                            m1 = fminf(e2, e3);
+                            const unsigned a = seg_admit(g.y, g.z, g.w, thr, py0, m0, m1);
+                            const unsigned f = seg_full(a, g.y, g.z, thr, py0, m0, m1);
+                            adm = a != 0u;
+                            done = done || f == 3u;
+                            m0 = (f & 1u) ? kSegAlways : (a & 1u) ? m0 : kSegNever;
+                            m1 = (f & 2u) ? kSegAlways : (a & 2u) ? m1 : kSegNever;
+                        }
+                        if (done) list[first + i] = id | kListDone;
+                        const unsigned bal = __ballot_sync(0xffffffffu, adm);
+                        uint32_t base = 0;
+                        if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
+                        base = __shfl_sync(0xffffffffu, base, 0);
+                        if (adm) {
+                            const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
+                            const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
+                            queue_put(sm, s, g.x, g.y, g.z, amp.x, amp.y, amp.z, m0, m1);
+                        }
                     }
                 }
                 __syncthreads();
