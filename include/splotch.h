@@ -141,6 +141,19 @@ int splotch_count_pairs(const splotch_particles *particles, int64_t n, const spl
                         const splotch_colormap *colormap, const splotch_params *params, void *workspace,
                         uint64_t workspace_bytes, uint64_t *pairs_host, uint64_t *visible_host, void *stream);
 
+/* Stage (b) of the paper's pipeline, "process data (e.g. for normalization)" (on the GPU
+ * "the processing involves normalizing of some particle values"): map a scalar field
+ * (the colval or I array) to [0, 1] by its own range before splotch_render (reading R17):
+ *     out[k] = clamp((f(values[k]) - lo) / (hi - lo), 0, 1),   f(v) = v or log10(v) (log_scale != 0),
+ * lo / hi = min / max of f over the values where f is defined and finite.  Where it is not (NaN, inf,
+ * v <= 0 under log10) out[k] = NaN, which splotch_render culls; hi == lo gives 0.
+ * splotch_field_range writes (lo, hi) to `range` (device, 2 floats; (0, 0) when no value is in the
+ * domain); splotch_field_normalize reads it from there.  Both only enqueue on `stream`; values and out
+ * are device arrays of n floats (out may equal values), caller-owned. */
+int splotch_field_range(const float *values, int64_t n, int32_t log_scale, float *range, void *stream);
+int splotch_field_normalize(const float *values, int64_t n, int32_t log_scale, const float *range, float *out,
+                            void *stream);
+
 /* out[k] = 1 - exp(-S[k]) for k < n_values (the additive output map, reading R13); S may
  * equal out.  Exposed for the multi-GPU path, which sums raw S images before this step. */
 int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream);

@@ -203,5 +203,24 @@ def render(w, camera=None, mode: Optional[int] = None, roi: Optional[Sequence[in
     return (out, int(nth.value)) if return_threads else out
 
 
+def normalize_field(values, log_scale: bool = False):
+    """Stage (b) of the paper's pipeline, "process data (e.g. for normalization)", reading R17
+    of DESIGN.md, written out in float64: f = identity or log10; lo / hi = min / max of f over the values where f
+    is defined and finite; out = clamp((f - lo) / (hi - lo), 0, 1), NaN where f is undefined, 0 when hi == lo.
+    Returns (out, (lo, hi)); (lo, hi) = (0, 0) when no value is in the domain."""
+    v = np.asarray(values, np.float64)
+    ok = np.isfinite(v)
+    if log_scale:
+        ok &= v > 0
+    f = np.full(v.shape, np.nan)
+    f[ok] = np.log10(v[ok]) if log_scale else v[ok]
+    if not ok.any():
+        return f, (0.0, 0.0)
+    lo, hi = float(f[ok].min()), float(f[ok].max())
+    out = np.full(v.shape, np.nan)
+    out[ok] = 0.0 if hi == lo else np.clip((f[ok] - lo) / (hi - lo), 0.0, 1.0)
+    return out, (lo, hi)
+
+
 def max_threads() -> int:
     return int(_load().orc_max_threads())

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libsplotch_b200.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "project.cu", "bin.cu", "scan.cu", "sort.cu", "raster_add.cu", "raster_mma.cu", "raster_abs.cu"]
+SOURCES = ["api.cu", "project.cu", "bin.cu", "scan.cu", "sort.cu", "raster_add.cu", "raster_mma.cu", "raster_abs.cu", "field.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 

@@ -448,6 +448,18 @@ int splotch_count_pairs(const splotch_particles *particles, int64_t n, const spl
     return splotch_workspace_status(workspace, stream, nullptr, visible_host, pairs_host);
 }
 
+int splotch_field_range(const float *values, int64_t n, int32_t log_scale, float *range, void *stream)
+{
+    if (n < 0 || !range || (n > 0 && !values)) return SPLOTCH_ERR_INVALID_ARG;
+    return launch_field_range(values, n, log_scale != 0, range, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int splotch_field_normalize(const float *values, int64_t n, int32_t log_scale, const float *range, float *out, void *stream)
+{
+    if (n < 0 || !range || (n > 0 && (!values || !out))) return SPLOTCH_ERR_INVALID_ARG;
+    return launch_field_normalize(values, n, log_scale != 0, range, out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream)
 {
     if (n_values < 0 || (n_values > 0 && (!S || !out))) return SPLOTCH_ERR_INVALID_ARG;

@@ -179,6 +179,9 @@ int launch_merge_absorb(const float *partials, const uint32_t *unit_prefix, cons
                         const CameraConst &cam, float *out, const WorkHead *head, cudaStream_t st);
 int launch_count_tensor_updates(const SplatAdd *records, int64_t n, const RenderConst &rc, const CameraConst &cam,
                                 WorkHead *head, cudaStream_t st);
+// field.cu: stage (b), range normalisation of a scalar field
+int launch_field_range(const float *v, int64_t n, int log_scale, float *range, cudaStream_t st);
+int launch_field_normalize(const float *v, int64_t n, int log_scale, const float *range, float *out, cudaStream_t st);
 int launch_normalize(const float *S, float *out, int64_t n_values, cudaStream_t st);
 
 }  // namespace splotch

@@ -384,3 +384,34 @@ def test_render_host_matches_device_render(B):
     np.testing.assert_allclose(out_host.numpy(), dev, rtol=2e-6, atol=1e-7)
     ref = oracle.render(w)
     _tol_check(out_host.numpy(), ref, "render_host")
+
+
+# ------------------------------------------------------------------------------------------------
+# stage (b): range normalisation of a scalar field on the device
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("log_scale", [False, True])
+@pytest.mark.parametrize("n", [0, 1, 3, 1025, 4_000_003])
+def test_field_normalisation_matches_oracle(B, n, log_scale):
+    rs = np.random.RandomState(n % 97 + 1)
+    v = rs.lognormal(-1.0, 2.5, n).astype(np.float32) - (0.0 if log_scale else 0.7)
+    if n >= 1025:
+        v[[7, 300, 1024]] = [np.nan, np.inf, -np.inf]
+        v[11] = 0.0
+        v[12] = -3.0
+    ref, (lo, hi) = oracle.normalize_field(v, log_scale)
+    buf = torch.empty(n + 1, dtype=torch.float32, device="cuda")          # +1: misaligned view exercises the scalar path
+    for view in (buf[:n], buf[1:n + 1]):
+        view.copy_(torch.from_numpy(v))
+        rng_dev = torch.empty(2, dtype=torch.float32, device="cuda")
+        out = torch.empty(n, dtype=torch.float32, device="cuda")
+        B.splotch_field_range(view, n, log_scale, rng_dev)
+        B.splotch_field_normalize(view, n, log_scale, rng_dev, out)
+        torch.cuda.synchronize()
+        got_rng = rng_dev.cpu().numpy().astype(np.float64)
+        np.testing.assert_allclose(got_rng, (lo, hi), rtol=2e-6, atol=2e-6)
+        got = out.cpu().numpy().astype(np.float64)
+        assert np.array_equal(np.isnan(got), np.isnan(ref))
+        np.testing.assert_allclose(got[~np.isnan(ref)], ref[~np.isnan(ref)], rtol=0, atol=3e-6)
+        B.splotch_field_normalize(view, n, log_scale, rng_dev, view)       # in place
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(view.cpu().numpy(), out.cpu().numpy())

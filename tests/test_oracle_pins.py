@@ -372,3 +372,40 @@ def test_absorb_zero_absorption_channel_is_pure_emission():
     np.testing.assert_allclose(out[:, :, 0], raw[:, :, 0], rtol=1e-13)
     np.testing.assert_allclose(out[:, :, 2], raw[:, :, 2], rtol=1e-13)
     assert np.all(out[:, :, 1] <= raw[:, :, 1] + 1e-15) and np.abs(out[:, :, 1] - raw[:, :, 1]).max() > 1e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# stage (b): range normalisation of a scalar field (reading R17)
+# ------------------------------------------------------------------------------------------------
+def test_p14_field_normalisation_closed_forms():
+    """Pins by construction: an arithmetic progression maps to k/(n-1); a geometric progression maps to k/(n-1)
+    under log10 (not under the identity); the map is invariant under v -> a v + b (a > 0) resp. v -> a v; undefined
+    values give NaN and do not move the range; a constant field gives 0."""
+    n = 11
+    k = np.arange(n) / (n - 1)
+    out, (lo, hi) = oracle.normalize_field(3.0 + 0.25 * np.arange(n))
+    np.testing.assert_allclose(out, k, atol=1e-15)
+    assert (lo, hi) == (3.0, 5.5)
+    geo = 1e-3 * 10.0 ** (0.5 * np.arange(n))
+    out, (lo, hi) = oracle.normalize_field(geo, log_scale=True)
+    np.testing.assert_allclose(out, k, atol=1e-14)
+    np.testing.assert_allclose((lo, hi), (-3.0, 2.0), atol=1e-14)
+    assert np.abs(oracle.normalize_field(geo)[0][1:-1] - k[1:-1]).min() > 0.05      # the identity map is a different function
+    rs = np.random.RandomState(3)
+    v = rs.lognormal(0.0, 2.0, 1000)
+    np.testing.assert_allclose(oracle.normalize_field(7.0 * v - 2.0)[0], oracle.normalize_field(v)[0], atol=1e-12)
+    np.testing.assert_allclose(oracle.normalize_field(7.0 * v, True)[0], oracle.normalize_field(v, True)[0], atol=1e-12)
+    w = v.copy()
+    w[[5, 17]] = [np.nan, np.inf]
+    out, rng_ = oracle.normalize_field(w)
+    assert np.isnan(out[[5, 17]]).all() and np.isfinite(np.delete(out, [5, 17])).all()
+    assert rng_ == oracle.normalize_field(np.delete(v, [5, 17]))[1]
+    w = v.copy()
+    w[[1, 2]] = [0.0, -4.0]
+    out, rng_ = oracle.normalize_field(w, True)
+    assert np.isnan(out[[1, 2]]).all() and out[np.argmax(w)] == 1.0 and np.nanmin(out) == 0.0
+    out, rng_ = oracle.normalize_field(np.full(9, 2.5))
+    assert (out == 0.0).all() and rng_ == (2.5, 2.5)
+    out, rng_ = oracle.normalize_field(np.array([np.nan, -1.0]), True)
+    assert np.isnan(out).all() and rng_ == (0.0, 0.0)
+    assert oracle.normalize_field(np.zeros(0))[1] == (0.0, 0.0)
