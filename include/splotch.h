@@ -154,6 +154,11 @@ int splotch_field_range(const float *values, int64_t n, int32_t log_scale, float
 int splotch_field_normalize(const float *values, int64_t n, int32_t log_scale, const float *range, float *out,
                             void *stream);
 
+/* The input of stage (d) "save the final image": 8-bit codes of an image written by
+ * splotch_render (reading R18): out[k] = rint(255 * clamp(rgb[k], 0, 1)^(1/gamma)), decided in fp32, NaN -> 0;
+ * gamma = 1 is the linear map.  rgb: device, n_values floats; out: device, n_values bytes; enqueue only. */
+int splotch_tonemap_rgb8(const float *rgb, int64_t n_values, float gamma, uint8_t *out, void *stream);
+
 /* out[k] = 1 - exp(-S[k]) for k < n_values (the additive output map, reading R13); S may
  * equal out.  Exposed for the multi-GPU path, which sums raw S images before this step. */
 int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream);

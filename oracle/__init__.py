@@ -222,5 +222,15 @@ def normalize_field(values, log_scale: bool = False):
     return out, (lo, hi)
 
 
+def tonemap_rgb8(values, gamma: float = 1.0):
+    """Reading R18: 8-bit code rint(255 * clamp(x, 0, 1)^(1/gamma)), NaN -> 0.  The integer is decided in fp32
+    (the kernel's precision): clamp, power and the product by 255 are float32 operations, rint is round-half-even."""
+    x = np.asarray(values, np.float32)
+    y = np.where(np.isnan(x), np.float32(0), np.clip(x, np.float32(0), np.float32(1))).astype(np.float32)
+    if gamma != 1.0:
+        y = np.power(y, np.float32(1.0) / np.float32(gamma), dtype=np.float32)
+    return np.rint(np.float32(255.0) * y).astype(np.uint8)
+
+
 def max_threads() -> int:
     return int(_load().orc_max_threads())

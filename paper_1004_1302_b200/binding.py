@@ -31,7 +31,7 @@ SPLOTCH_FORCE_TENSOR = 4
 # every symbol include/splotch.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
     "splotch_workspace_bytes", "splotch_render", "splotch_workspace_status", "splotch_count_pairs",
-    "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
+    "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_tonemap_rgb8", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
     "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_tensor_stats", "splotch_debug_scan",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
     "splotch_last_cuda_error", "splotch_version", "splotch_profile_enable", "splotch_profile_read",
@@ -227,6 +227,11 @@ def splotch_field_normalize(values, n: int, log_scale: bool, range_in, out, stre
     _check("splotch_field_normalize",
            _lib().splotch_field_normalize(_vp(_ptr(values)), C.c_int64(n), C.c_int32(1 if log_scale else 0),
                                           _vp(_ptr(range_in)), _vp(_ptr(out)), _vp(_stream(stream))))
+
+
+def splotch_tonemap_rgb8(rgb, n_values: int, gamma: float, out, stream=None) -> None:
+    _check("splotch_tonemap_rgb8", _lib().splotch_tonemap_rgb8(_vp(_ptr(rgb)), C.c_int64(n_values), C.c_float(gamma),
+                                                             _vp(_ptr(out)), _vp(_stream(stream))))
 
 
 def splotch_render_host(particles_host: splotch_particles, n: int, camera: splotch_camera,

@@ -460,6 +460,12 @@ int splotch_field_normalize(const float *values, int64_t n, int32_t log_scale, c
     return launch_field_normalize(values, n, log_scale != 0, range, out, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int splotch_tonemap_rgb8(const float *rgb, int64_t n_values, float gamma, uint8_t *out, void *stream)
+{
+    if (n_values < 0 || !(gamma > 0.0f) || (n_values > 0 && (!rgb || !out))) return SPLOTCH_ERR_INVALID_ARG;
+    return launch_tonemap_rgb8(rgb, n_values, gamma, out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream)
 {
     if (n_values < 0 || (n_values > 0 && (!S || !out))) return SPLOTCH_ERR_INVALID_ARG;

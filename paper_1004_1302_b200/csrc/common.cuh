@@ -182,6 +182,7 @@ int launch_count_tensor_updates(const SplatAdd *records, int64_t n, const Render
 // field.cu: stage (b), range normalisation of a scalar field
 int launch_field_range(const float *v, int64_t n, int log_scale, float *range, cudaStream_t st);
 int launch_field_normalize(const float *v, int64_t n, int log_scale, const float *range, float *out, cudaStream_t st);
+int launch_tonemap_rgb8(const float *v, int64_t n, float gamma, uint8_t *out, cudaStream_t st);
 int launch_normalize(const float *S, float *out, int64_t n_values, cudaStream_t st);
 
 }  // namespace splotch

@@ -104,6 +104,32 @@ field_normalize_kernel(const float *__restrict__ v, long long n, int log_scale, 
     for (long long i = done + t0; i < n; i += stride) out[i] = map_one(__ldg(v + i), log_scale, lo, span);
 }
 
+// Stage (d) input ("save the final image"): 8-bit code of an image value, reading R18:
+// code = rint(255 * clamp(x, 0, 1)^(1/gamma)), NaN -> 0; fp32 throughout (the integer is decided in fp32).
+__device__ __forceinline__ unsigned tone_one(float x, float inv_gamma)
+{
+    float y = fminf(fmaxf(x, 0.0f), 1.0f);          // fmaxf(NaN, 0) = 0
+    if (inv_gamma != 1.0f) y = powf(y, inv_gamma);
+    return (unsigned)__float2int_rn(__fmul_rn(255.0f, y));
+}
+
+__global__ void __launch_bounds__(kFieldThreads)
+tonemap_rgb8_kernel(const float *__restrict__ v, long long n, float inv_gamma, uint8_t *__restrict__ out, int vec_ok)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x, t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long done = 0;
+    if (vec_ok) {
+        const long long n4 = n >> 2;
+        for (long long i = t0; i < n4; i += stride) {
+            const float4 q = __ldg(reinterpret_cast<const float4 *>(v) + i);
+            reinterpret_cast<uint32_t *>(out)[i] = tone_one(q.x, inv_gamma) | (tone_one(q.y, inv_gamma) << 8) |
+                                                   (tone_one(q.z, inv_gamma) << 16) | (tone_one(q.w, inv_gamma) << 24);
+        }
+        done = n4 << 2;
+    }
+    for (long long i = done + t0; i < n; i += stride) out[i] = (uint8_t)tone_one(__ldg(v + i), inv_gamma);
+}
+
 unsigned field_grid(int64_t n)
 {
     long long blocks = (n / 4 + kFieldThreads - 1) / kFieldThreads + 1;
@@ -124,6 +150,15 @@ int launch_field_range(const float *v, int64_t n, int log_scale, float *range, c
         SPLOTCH_LAUNCH_CHECK();
     }
     field_range_finish_kernel<<<1, 1, 0, st>>>(code, log_scale);
+    SPLOTCH_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_tonemap_rgb8(const float *v, int64_t n, float gamma, uint8_t *out, cudaStream_t st)
+{
+    if (n <= 0) return 0;
+    const int vec_ok = (reinterpret_cast<uintptr_t>(v) & 15u) == 0 && (reinterpret_cast<uintptr_t>(out) & 3u) == 0;
+    tonemap_rgb8_kernel<<<field_grid(n), kFieldThreads, 0, st>>>(v, (long long)n, 1.0f / gamma, out, vec_ok);
     SPLOTCH_LAUNCH_CHECK();
     return 0;
 }

@@ -18,7 +18,7 @@ def lib():
 def _declared():
     text = open(os.path.join(ROOT, "include", "splotch.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(splotch_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(splotch_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported(lib):

@@ -409,3 +409,16 @@ def test_p14_field_normalisation_closed_forms():
     out, rng_ = oracle.normalize_field(np.array([np.nan, -1.0]), True)
     assert np.isnan(out).all() and rng_ == (0.0, 0.0)
     assert oracle.normalize_field(np.zeros(0))[1] == (0.0, 0.0)
+
+
+def test_p15_tonemap_codes():
+    """Pins: the codes of k/255 are k; values below 0 / above 1 / NaN clamp to 0 / 255 / 0; halves round to even;
+    gamma 2 maps (k/255)^2 back to k; the map is monotone."""
+    k = np.arange(256)
+    assert np.array_equal(oracle.tonemap_rgb8(k / 255.0), k)
+    assert list(oracle.tonemap_rgb8([-1.0, 0.0, 1.0, 7.0, np.nan, np.inf, -np.inf])) == [0, 0, 255, 255, 0, 255, 0]
+    assert list(oracle.tonemap_rgb8(np.array([0.5, 1.5, 2.5, 3.5]) / 255.0)) == [0, 2, 2, 4]
+    assert np.array_equal(oracle.tonemap_rgb8((k / 255.0) ** 2, gamma=2.0), k)
+    x = np.sort(np.random.RandomState(1).uniform(-0.2, 1.2, 5000))
+    for g in (1.0, 2.2):
+        assert (np.diff(oracle.tonemap_rgb8(x, g).astype(int)) >= 0).all()
