@@ -75,12 +75,17 @@ __device__ __forceinline__ void splat_tile(const float *__restrict__ gxs, const 
     }
 }
 
+// kMma: the tensor-core kernel has run before on the same lists (handled segments and finished list entries are
+// skipped here); !kMma: every covered pixel is accumulated here.  With tensor == 2 both instantiations are launched
+// and the one that does not match the device-side choice returns at once.
+template <bool kMma>
 __global__ void __launch_bounds__(kRasThreads, 2)
 raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__restrict__ list,
                        const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
                        int nbx, int W, int H, float thr, float *__restrict__ S, WorkHead *head, int vec_ok, int tensor)
 {
-    const int mma_on = tensor == 2 ? (int)head->tensor_on : tensor;
+    constexpr bool mma_on = kMma;
+    if (tensor == 2 && (head->tensor_on != 0u) != kMma) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SmemAdd &sm = *reinterpret_cast<SmemAdd *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -113,7 +118,11 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
         // ids of the unit, without the entries the tensor-core kernel marked as finished
         if (tid == 0) sm.n_ids = 0u;
         __syncthreads();
-        for (uint32_t i0 = 0; i0 < unit_count; i0 += kRasThreads) {
+        if (!kMma) {
+            for (uint32_t i = tid; i < unit_count; i += kRasThreads) sm.ids[i] = __ldg(list + first + i);
+            if (tid == 0) sm.n_ids = unit_count;
+        }
+        for (uint32_t i0 = 0; kMma && i0 < unit_count; i0 += kRasThreads) {
             const uint32_t i = i0 + tid;
             const uint32_t id = i < unit_count ? __ldg(list + first + i) : kListDone;
             const bool keep = !(id & kListDone);
@@ -143,6 +152,10 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
             const int s = tid >> 3, part = tid & 7;
             const uint32_t e = (uint32_t)b * kBatch + s;
             const bool valid = b < n_batches && e < count;
+            if (!kMma && !valid) {                  // no shuffles in this instantiation: lanes without a splat may leave
+                *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = 0;
+                return;
+            }
             float4 g = make_float4(0.f, 0.f, 0.f, 0.f), a = g;
             if (valid) {
                 g = *reinterpret_cast<const float4 *>(&sm.rec[slot][s]);        // sx, sy, c, R
@@ -320,14 +333,23 @@ int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const 
 {
     static bool attr_set = false;
     if (!attr_set) {
-        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)sizeof(SmemAdd)));
+        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               (int)sizeof(SmemAdd)));
         attr_set = true;
     }
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
-    raster_additive_kernel<<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(
-        records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);
-    SPLOTCH_LAUNCH_CHECK();
+    if (tensor != 0) {
+        raster_additive_kernel<true><<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(
+            records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);
+        SPLOTCH_LAUNCH_CHECK();
+    }
+    if (tensor != 1) {
+        raster_additive_kernel<false><<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(
+            records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);
+        SPLOTCH_LAUNCH_CHECK();
+    }
     return 0;
 }
 
