@@ -2,7 +2,7 @@
 //
 // One CTA (8 warps) owns a 64x64-pixel block of the screen for the duration of a work unit (a
 // chunk of that block's splat list).  The block is cut into sixteen 16x16 tiles; every warp owns
-// TWO of them, far apart ((tx + 2 ty) mod 8 == warp), so that the compact cluster of tiles a splat
+// TWO of them, far apart (tile (tx, ty) with tx < 2 and (tx + 2, (ty + 1) mod 4)), so that the compact cluster of tiles a splat
 // touches spreads over many warps.  A lane owns 8 consecutive pixels of one tile row in each of
 // its two tiles: 48 accumulators in REGISTERS, held as 24 packed f32x2 pairs.
 // Per batch of 32 splats the CTA
@@ -25,8 +25,13 @@ namespace {
 
 constexpr int kRasThreads = 256;
 constexpr int kTiles = 16;                      // 16x16-pixel tiles of a block, index ty * 4 + tx
-constexpr uint32_t kTileA = 0xBA763210u;        // nibble w: first tile of warp w  ((tx + 2 ty) mod 8 == w)
-constexpr uint32_t kTileB = 0xDC9854FEu;        // nibble w: second tile of warp w
+// Tiles of warp w (nibble w): (tx, ty) with tx < 2 and its partner (tx + 2, (ty + 1) mod 4): no row, column or diagonal
+// of tiles and no 2x2 cluster holds both tiles of a warp, so a splat rarely gives a warp two items in one batch (the warps
+// meet at a barrier after every batch).  Measured K3 time on C3 for the partner rule: (tx+2, ty+1) 239.8 ms, (tx+2, ty+2)
+// 241.9, point-symmetric (15 - t) 243.4, (tx + 2 ty) mod 8 == w 247.8, (tx+1, ty+2) 250.2; pairing the heaviest tile of a
+// block (by the work its earlier units saw) with the lightest one 247.1: the spread inside a batch counts, not the totals.
+constexpr uint32_t kTileA = 0xDC985410u;
+constexpr uint32_t kTileB = 0x32FEBA76u;
 
 struct SmemAdd {
     float4 row[2][kBatch][kBlockPx];            // (a_r gy, a_g gy, a_b gy, thr / gy) per splat and block row
