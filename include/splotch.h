@@ -67,6 +67,12 @@ typedef struct {
     const float *I;           /* optical-depth modulation = rho_0p (last sentence) */
     const float *colval;      /* scalar mapped through the colour table, clamped to [0, 1]    */
     const uint8_t *type;      /* particle type 0..n_types-1; NULL means all type 0            */
+    /* Optional vector colouring ("the three components of the vectors can be mapped to the three
+     * components of E and A"; reading R19): when vr is not NULL, vr / vg / vb (length n, all three required) give
+     * E_p = brightness[type] * (vr, vg, vb) and A_p = abs_brightness[type] * (vr, vg, vb) directly, used as given
+     * (no clamp); colval and the colour tables are ignored (colval may then be NULL); a particle with a non-finite
+     * component is culled.  Zero-initialise the struct to keep the scalar path. */
+    const float *vr, *vg, *vb;
 } splotch_particles;
 
 /* Pinhole perspective camera (reading R1, R2): fwd = normalise(lookat - eye),
@@ -167,7 +173,8 @@ int splotch_normalize(const float *S, float *out, int64_t n_values, void *stream
  * device (staging areas inside `workspace`), renders, copies the image back to
  * `out_rgb_host` and SYNCHRONISES.  All pointers inside `particles_host` and
  * `colormap_host` and `out_rgb_host` are host pointers (pinned memory gives the best copy
- * rate).  workspace must be at least splotch_workspace_bytes_host(...) bytes of device memory. */
+ * rate).  workspace must be at least splotch_workspace_bytes_host(...) bytes of device memory.
+ * Scalar colouring only: particles_host->vr must be NULL. */
 int splotch_workspace_bytes_host(int64_t n, const splotch_camera *camera, const splotch_colormap *colormap_host,
                                  const splotch_params *params, uint64_t max_pairs, uint64_t *bytes);
 

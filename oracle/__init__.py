@@ -203,6 +203,36 @@ def render(w, camera=None, mode: Optional[int] = None, roi: Optional[Sequence[in
     return (out, int(nth.value)) if return_threads else out
 
 
+def render_vector(w, camera=None, mode: Optional[int] = None, roi: Optional[Sequence[int]] = None, raw: bool = False):
+    """Vector colouring ("the three components of the vectors can be mapped to the three components of
+    E and A"; reading R19): E_p = brightness[type] * v_p, A_p = abs_brightness[type] * v_p with v_p = w.vec[p] used as
+    given; a particle with a non-finite component is culled.  Stage 1 is the pinned splat table evaluated with colour
+    tables that are identically one (so that its E / A columns hold the brightness of the particle's type), scaled here
+    by the vector in float64; stage 2 is render_table."""
+    camera = camera or w.camera
+    mode = w.mode if mode is None else mode
+    vec = np.asarray(w.vec, np.float64)
+    ones = np.ones((int(w.lut_e.shape[0]), 2, 3), np.float32)
+    import copy
+    w1 = copy.copy(w)
+    w1.lut_e, w1.lut_a = ones, ones
+    w1.colval = np.zeros(len(vec), np.float32)
+    table, ok = splat_table(w1, camera, mode)
+    fin = np.isfinite(vec).all(axis=1)
+    table = table.copy()
+    table[:, 5:8] *= np.where(fin[:, None], vec, 0.0)
+    table[:, 8:11] *= np.where(fin[:, None], vec, 0.0)
+    ok = ok.astype(bool) & fin
+    if mode == 0:
+        seq = np.nonzero(ok)[0]
+    else:
+        p = project_f32(w1, camera)
+        seq = depth_order(p["zkey"], (p["visible"].astype(bool) & fin).astype(np.uint8))
+    if roi is None:
+        roi = (0, 0, camera.width, camera.height)
+    return render_table(table, seq, mode, roi, raw)
+
+
 def normalize_field(values, log_scale: bool = False):
     """Stage (b) of the paper's pipeline, "process data (e.g. for normalization)", reading R17
     of DESIGN.md, written out in float64: f = identity or log10; lo / hi = min / max of f over the values where f

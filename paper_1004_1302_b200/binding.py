@@ -50,7 +50,7 @@ class SplotchError(RuntimeError):
 
 class splotch_particles(C.Structure):
     _fields_ = [("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p), ("r", C.c_void_p), ("I", C.c_void_p),
-                ("colval", C.c_void_p), ("type", C.c_void_p)]
+                ("colval", C.c_void_p), ("type", C.c_void_p), ("vr", C.c_void_p), ("vg", C.c_void_p), ("vb", C.c_void_p)]
 
 
 class splotch_camera(C.Structure):
@@ -113,8 +113,11 @@ def _stream(stream) -> Optional[int]:
     return int(stream.cuda_stream)
 
 
-def make_particles(x, y, z, r, I, colval, type=None) -> splotch_particles:
-    return splotch_particles(_ptr(x), _ptr(y), _ptr(z), _ptr(r), _ptr(I), _ptr(colval), _ptr(type))
+def make_particles(x, y, z, r, I, colval, type=None, vec=None) -> splotch_particles:
+    """vec: optional (vr, vg, vb) arrays for vector colouring (colval may then be None)."""
+    v = (None, None, None) if vec is None else vec
+    return splotch_particles(_ptr(x), _ptr(y), _ptr(z), _ptr(r), _ptr(I), _ptr(colval), _ptr(type),
+                             _ptr(v[0]), _ptr(v[1]), _ptr(v[2]))
 
 
 def make_camera(eye: Sequence[float], lookat: Sequence[float], up: Sequence[float], fov_deg: float, width: int,

@@ -127,7 +127,9 @@ int check_particles(const splotch_particles *p, int64_t n)
 {
     if (n < 0) return SPLOTCH_ERR_INVALID_ARG;
     if (n >= (1ll << 31)) return SPLOTCH_ERR_LIMIT;
-    if (n > 0 && (!p || !p->x || !p->y || !p->z || !p->r || !p->I || !p->colval)) return SPLOTCH_ERR_INVALID_ARG;
+    if (n > 0 && (!p || !p->x || !p->y || !p->z || !p->r || !p->I)) return SPLOTCH_ERR_INVALID_ARG;
+    if (n > 0 && p->vr && (!p->vg || !p->vb)) return SPLOTCH_ERR_INVALID_ARG;
+    if (n > 0 && !p->vr && !p->colval) return SPLOTCH_ERR_INVALID_ARG;
     return SPLOTCH_OK;
 }
 
@@ -230,8 +232,9 @@ int run_front(const Ctx &c, const splotch_particles *particles, int64_t n, const
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.head, 0, 256, c.st));
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_count, 0, (size_t)c.n_bins * 4, c.st));
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_cursor, 0, (size_t)c.n_bins * 4, c.st));
-    ParticlePtrs pp = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
-    if (n > 0) pp = { particles->x, particles->y, particles->z, particles->r, particles->I, particles->colval, particles->type };
+    ParticlePtrs pp = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
+    if (n > 0) pp = { particles->x, particles->y, particles->z, particles->r, particles->I, particles->colval, particles->type,
+                      particles->vr, particles->vg, particles->vb };
     int rc = launch_project(pp, n, c.cam, c.rc, cm->emission, cm->absorption, c.ws + c.L.records,
                             c.at<uint32_t>(c.L.bin_count), c.rc.mode == SPLOTCH_ABSORB ? c.at<uint32_t>(c.L.zkeys) : nullptr,
                             c.head(), dbg, c.st);
@@ -515,6 +518,7 @@ int splotch_render_host(const splotch_particles *ph, int64_t n, const splotch_ca
                         void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream)
 {
     if (!out_rgb_host || !workspace || !params) return SPLOTCH_ERR_INVALID_ARG;
+    if (ph && (ph->vr || !ph->colval) && n > 0) return SPLOTCH_ERR_INVALID_ARG;     // host path: scalar colouring only
     int rc = check_particles(ph, n);
     if (rc) return rc;
     rc = check_colormap(cmh, params->mode);

@@ -118,6 +118,7 @@ int sm_count();
 struct ParticlePtrs {
     const float *x, *y, *z, *r, *I, *colval;
     const uint8_t *type;
+    const float *vr, *vg, *vb;      // optional vector colouring (reading R19)
 };
 
 struct DebugProjectOut {

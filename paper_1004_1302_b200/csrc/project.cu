@@ -141,7 +141,7 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
             const float4 c = __ldg(reinterpret_cast<const float4 *>(p.z) + g);
             const float4 d = __ldg(reinterpret_cast<const float4 *>(p.r) + g);
             const float4 e = __ldg(reinterpret_cast<const float4 *>(p.I) + g);
-            const float4 f = __ldg(reinterpret_cast<const float4 *>(p.colval) + g);
+            const float4 f = p.colval ? __ldg(reinterpret_cast<const float4 *>(p.colval) + g) : make_float4(0.f, 0.f, 0.f, 0.f);
             xv[0] = a.x; xv[1] = a.y; xv[2] = a.z; xv[3] = a.w;
             yv[0] = b.x; yv[1] = b.y; yv[2] = b.z; yv[3] = b.w;
             zv[0] = c.x; zv[1] = c.y; zv[2] = c.z; zv[3] = c.w;
@@ -164,7 +164,7 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
                 zv[k] = in ? __ldg(p.z + i) : 0.0f;
                 rv[k] = in ? __ldg(p.r + i) : -1.0f;      // r <= 0: culled
                 Iv[k] = in ? __ldg(p.I + i) : 0.0f;
-                cvv[k] = in ? __ldg(p.colval + i) : 0.0f;
+                cvv[k] = (in && p.colval) ? __ldg(p.colval + i) : 0.0f;
                 tv[k] = (in && p.type) ? (int)__ldg(p.type + i) : 0;
             }
         }
@@ -172,6 +172,11 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
         for (int k = 0; k < 4; ++k) {
             const long long i = base + k;
             const bool in = g < groups && i < n;
+            float v0 = 0.0f, v1 = 0.0f, v2 = 0.0f;
+            if (p.vr) {                          // vector colouring (reading R19): a non-finite component culls the particle
+                if (in) { v0 = __ldg(p.vr + i); v1 = __ldg(p.vg + i); v2 = __ldg(p.vb + i); }
+                cvv[k] = (finite_f(v0) && finite_f(v1) && finite_f(v2)) ? 0.0f : __int_as_float(0x7fc00000);
+            }
             const Projected o = project_one(xv[k], yv[k], zv[k], rv[k], Iv[k], cvv[k], tv[k], cam, rc);
             const uint32_t bins = o.visible ? pack_bins(o, rc.bin_shift) : kInvisible;
             if (in) {
@@ -184,14 +189,20 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
                 const float tau0 = (Iv[k] * rv[k]) * kSqrtPi;
                 const float cw = o.visible ? kSqrtLog2e / o.ss : 0.0f;
                 float er = 0.f, eg = 0.f, eb = 0.f;
-                if (o.visible) lut_sample(lutE, rc.n_entries, tv[k], cvv[k], rc.brightness[tv[k]], er, eg, eb);
+                if (o.visible) {
+                    if (p.vr) { const float sc = rc.brightness[tv[k]]; er = sc * v0; eg = sc * v1; eb = sc * v2; }
+                    else lut_sample(lutE, rc.n_entries, tv[k], cvv[k], rc.brightness[tv[k]], er, eg, eb);
+                }
                 if (!kAbsorb) {
                     float4 *rec = reinterpret_cast<float4 *>(reinterpret_cast<SplatAdd *>(records) + i);
                     rec[0] = make_float4(o.sx, o.sy, cw, o.R);
                     rec[1] = make_float4(er * tau0, eg * tau0, eb * tau0, __uint_as_float(bins));
                 } else {
                     float ar = 0.f, ag = 0.f, ab = 0.f;
-                    if (o.visible) lut_sample(lutA, rc.n_entries, tv[k], cvv[k], rc.abs_brightness[tv[k]], ar, ag, ab);
+                    if (o.visible) {
+                        if (p.vr) { const float sc = rc.abs_brightness[tv[k]]; ar = sc * v0; ag = sc * v1; ab = sc * v2; }
+                        else lut_sample(lutA, rc.n_entries, tv[k], cvv[k], rc.abs_brightness[tv[k]], ar, ag, ab);
+                    }
                     float4 *rec = reinterpret_cast<float4 *>(reinterpret_cast<SplatAbs *>(records) + i);
                     rec[0] = make_float4(o.sx, o.sy, cw, o.R);
                     rec[1] = make_float4(o.visible ? tau0 : 0.0f, er, eg, eb);

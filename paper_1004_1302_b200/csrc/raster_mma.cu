@@ -14,13 +14,11 @@
 //
 // The contraction runs as tcgen05.mma kind::tf32 (M = 128, N = 64, K = 8) with A in tensor memory
 // (written by the producing warps with tcgen05.st), B in shared memory (K-major, no swizzle) and the
-// fp32 accumulators D_0, D_1 in tensor memory.  Precision: every operand is split into two TF32 numbers
-// (hi = rna(v), lo = rna(v - hi)) and three products are accumulated (hi*hi + lo*hi + hi*lo), which
-// leaves a relative error of ~2^-21 per term instead of 2^-11 -- fp32 class, inside the 1e-4 parity
-// tolerance for any amplitude.
-//
-// The split is computed with integer arithmetic on the fp32 bits (hi = (bits + 0x1000) & ~0x1fff, i.e.
-// round to nearest, ties away; lo = v - hi exactly; the tensor core ignores the 13 low bits of lo).
+// fp32 accumulators D_0, D_1 in tensor memory.  Precision: every operand is split into two numbers,
+// v = hi + lo with hi a TF32 number (Veltkamp split with 2^13 + 1 in packed f32x2 arithmetic: hi has 11
+// significant bits, lo = v - hi exactly; the tensor core ignores the 13 low bits of lo), and three
+// products are accumulated (hi*hi + lo*hi + hi*lo), which leaves a relative error of ~2^-21 per term
+// instead of 2^-11 -- fp32 class, inside the 1e-4 parity tolerance for any amplitude.
 //
 // One CTA (11 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
 // kUnitsPerTicket consecutive work units of its splat list:
@@ -50,8 +48,8 @@ constexpr int kPerThread = 2;             // list entries per filter thread and 
 constexpr int kFilterChunk = kFilterThreads * kPerThread;   // list entries per filter pass
 constexpr int kQueue = 1024;              // ring of admitted splats (power of two, > kFilterChunk + a batch)
 // The tensor core adds every K = 8 dot product into the fp32 accumulator with truncation: a relative deficit of
-// ~2^-25 per MMA (measured on C3: -7e-5 with 8 units = ~3700 MMAs per accumulator between flushes).  Two units
-// (~900 MMAs) keep it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
+// ~2^-25 per MMA (measured on C3: -7e-5 with ~3700 MMAs per accumulator between flushes).  One unit of 4096 list
+// entries (~900 MMAs) keeps it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
 constexpr int kUnitsPerTicket = 1;
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
@@ -129,13 +127,6 @@ __device__ __forceinline__ uint64_t b_descriptor(const float *b)
 }
 
 constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kBlockPx >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-
-// v = hi + lo with hi a TF32 number (round to nearest, ties away) and lo = v - hi exact in fp32
-__device__ __forceinline__ void split_tf32(float v, uint32_t &hi, uint32_t &lo)
-{
-    hi = (__float_as_uint(v) + 0x1000u) & 0xffffe000u;
-    lo = __float_as_uint(__fsub_rn(v, __uint_as_float(hi)));
-}
 
 __device__ __forceinline__ void queue_put(SmemMma &sm, uint32_t s, float sx, float sy, float c, float ar, float ag, float ab,
                                           float m0, float m1)

@@ -34,6 +34,8 @@ class Scene:
         self.n_types, self.n_entries = int(w.lut_e.shape[0]), int(w.lut_e.shape[1])
         self._host = {k: np.ascontiguousarray(getattr(w, k), np.float32) for k in ("x", "y", "z", "r", "I", "colval")}
         self._host_type = None if w.type is None else np.ascontiguousarray(w.type, np.uint8)
+        vec = getattr(w, "vec", None)       # optional (n, 3) vector colouring
+        self._host_vec = None if vec is None else [np.ascontiguousarray(np.asarray(vec, np.float32)[:, k]) for k in range(3)]
         self._host_lut_e = np.ascontiguousarray(w.lut_e, np.float32)
         self._host_lut_a = None if w.lut_a is None else np.ascontiguousarray(w.lut_a, np.float32)
         self.d = {}
@@ -49,13 +51,14 @@ class Scene:
             for k, a in self._host.items():
                 self.d[k] = torch.from_numpy(a).to(self.device)
             self.d["type"] = None if self._host_type is None else torch.from_numpy(self._host_type).to(self.device)
+            self.d["vec"] = None if self._host_vec is None else [torch.from_numpy(a).to(self.device) for a in self._host_vec]
             self.d["lut_e"] = torch.from_numpy(self._host_lut_e).to(self.device)
             self.d["lut_a"] = None if self._host_lut_a is None else torch.from_numpy(self._host_lut_a).to(self.device)
             torch.cuda.synchronize(self.device)
 
     def particles(self) -> B.splotch_particles:
         d = self.d
-        return B.make_particles(d["x"], d["y"], d["z"], d["r"], d["I"], d["colval"], d["type"])
+        return B.make_particles(d["x"], d["y"], d["z"], d["r"], d["I"], d["colval"], d["type"], d["vec"])
 
     def colormap(self) -> B.splotch_colormap:
         return B.make_colormap(self.d["lut_e"], self.d["lut_a"], self.n_entries, self.n_types)

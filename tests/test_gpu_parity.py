@@ -436,3 +436,28 @@ def test_tonemap_codes_match_oracle(B, n, gamma):
         y = 255.0 * np.clip(np.nan_to_num(v.astype(np.float64), nan=0.0), 0, 1) ** (1.0 / gamma)   # flip only next to a half
         bad = got != ref
         assert (np.abs(got - ref) <= 1).all() and (np.abs((y[bad] % 1.0) - 0.5) < 1e-3).all() and bad.sum() <= 1e-3 * max(n, 1)
+
+
+# ------------------------------------------------------------------------------------------------
+# vector colouring (reading R19)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [ADDITIVE, ABSORB])
+def test_vector_colouring_matches_oracle(B, mode):
+    w = workloads.make("C1", 60_000, width=300, height=212)
+    rs = np.random.RandomState(21)
+    w.vec = rs.uniform(0.0, 1.5, (w.n, 3)).astype(np.float32)
+    w.vec[[5, 900], [0, 2]] = [np.nan, np.inf]                 # culled
+    w.mode = mode
+    if mode == ABSORB:
+        w.lut_a = w.lut_e.copy()                               # ignored, but the absorb mode wants a table
+        w.abs_brightness = [0.6 * b for b in w.brightness]
+    sc = _scene(w)
+    sc.d["colval"] = None                                      # colval may be NULL with vector colouring
+    out = sc.render(raw=(mode == ADDITIVE)).cpu().numpy()
+    ref = oracle.render_vector(w, raw=(mode == ADDITIVE))
+    assert ref.max() > 0.2
+    _tol_check(out, ref, f"vector colouring, mode {mode}")
+    # the colour table is really ignored: a different table gives the same image
+    w.lut_e = w.lut_e[:, ::-1].copy()
+    out2 = _scene(w).render(raw=(mode == ADDITIVE)).cpu().numpy()
+    np.testing.assert_allclose(out2, out, rtol=2e-5, atol=1e-6)

@@ -422,3 +422,38 @@ def test_p15_tonemap_codes():
     x = np.sort(np.random.RandomState(1).uniform(-0.2, 1.2, 5000))
     for g in (1.0, 2.2):
         assert (np.diff(oracle.tonemap_rgb8(x, g).astype(int)) >= 0).all()
+
+
+def test_p16_vector_colouring_reduces_to_the_scalar_path():
+    """PAPER.md:75 vector colouring (reading R19).  Pins: a constant vector is a constant colour table; in the additive
+    raw sum channel c with per-particle v_c equals the scalar path with a table of ones and I scaled by v_c (tau is
+    linear in I, O6); a particle with a non-finite component vanishes."""
+    import copy
+    rs = np.random.RandomState(7)
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=72, h=56)
+    n = 40
+    pts = np.stack([rs.uniform(-1.5, 1.5, n), rs.uniform(-1.2, 1.2, n), rs.uniform(-1, 1, n), rs.uniform(0.05, 0.4, n),
+                    rs.uniform(0.5, 2.0, n), rs.uniform(0, 1, n)], 1)
+    w = mk(pts, c, lut_e=const_lut((0.7, 0.4, 0.2)), brightness=(1.3,))
+    ref = oracle.render(w, raw=True)
+    wv = copy.copy(w)
+    wv.vec = np.tile(np.array([[0.7, 0.4, 0.2]], np.float32), (n, 1))
+    np.testing.assert_allclose(oracle.render_vector(wv, raw=True), ref, rtol=1e-12, atol=1e-15)
+    vec = rs.uniform(0.0, 2.0, (n, 3)).astype(np.float32)
+    wv.vec = vec
+    got = oracle.render_vector(wv, raw=True)
+    for ch in range(3):
+        w1 = mk(np.column_stack([pts[:, :4], pts[:, 4] * vec[:, ch].astype(np.float64), pts[:, 5]]), c, lut_e=const_lut(),
+                brightness=(1.3,))
+        # I is stored as float32 in the workload: compare at float32 resolution of the product
+        np.testing.assert_allclose(got[..., ch], oracle.render(w1, raw=True)[..., 0], rtol=3e-7, atol=1e-12)
+    wv.vec = vec.copy()
+    wv.vec[3, 1] = np.nan
+    keep = np.arange(n) != 3
+    w2 = mk(pts[keep], c, lut_e=const_lut(), brightness=(1.3,))
+    w2.vec = vec[keep]
+    np.testing.assert_allclose(oracle.render_vector(wv, raw=True), oracle.render_vector(w2, raw=True), rtol=1e-12, atol=1e-15)
+    # absorb mode: A = abs_brightness * v as well; with equal brightness this is the additive image (P7)
+    wa = mk(pts, c, lut_e=const_lut(), lut_a=const_lut(), brightness=(1.3,), abs_brightness=(1.3,), mode=ABSORB)
+    wa.vec = vec
+    np.testing.assert_allclose(oracle.render_vector(wa), oracle.render_vector(wv.__class__(**{**wv.__dict__, "vec": vec})), rtol=1e-9, atol=1e-12)

@@ -71,6 +71,7 @@ class Workload:
     support_f: float = 3.0
     z_near: float = 0.01
     notes: Dict[str, object] = field(default_factory=dict)
+    vec: Optional[np.ndarray] = None     # (n, 3) float32: vector colouring, replaces colval + tables
 
     @property
     def camera(self) -> Camera:
@@ -87,7 +88,8 @@ class Workload:
         arr = [np.ascontiguousarray(a[sl]) for a in (self.x, self.y, self.z, self.r, self.I, self.colval)]
         return Workload(self.name + f"/stride{stride}", len(arr[0]), self.seed, *arr, t, self.cameras,
                         self.lut_e, self.lut_a, list(self.brightness), list(self.abs_brightness),
-                        self.mode, self.support_f, self.z_near, dict(self.notes))
+                        self.mode, self.support_f, self.z_near, dict(self.notes),
+                        None if self.vec is None else np.ascontiguousarray(self.vec[sl]))
 
     def checksums(self) -> Dict[str, int]:
         out = {}
