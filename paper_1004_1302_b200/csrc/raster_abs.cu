@@ -34,6 +34,14 @@ __device__ __forceinline__ float phi_small(float u)   // (1 - exp(-u)) / u for u
     return fmaf(p, u, 1.0f);
 }
 
+__device__ __forceinline__ float phi_tiny(float u)    // the same for u < 0.03: error < u^4 / 120 < 7e-9
+{
+    float p = -1.0f / 24.0f;
+    p = fmaf(p, u, 1.0f / 6.0f);
+    p = fmaf(p, u, -0.5f);
+    return fmaf(p, u, 1.0f);
+}
+
 __global__ void __launch_bounds__(kRasThreads, 1)
 raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__restrict__ list,
                      const uint64_t *__restrict__ bin_offset, const uint32_t *__restrict__ unit_prefix, int n_bins,
@@ -120,9 +128,13 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
         produce(0, 0);
         __syncthreads();
 
-        float C[24], L[24];
+        // state per pixel and channel: colour C and transmittance T = exp(-L).  T is carried as a product, so the common
+        // case (every u = A tau of the splat below 0.25) needs no exponential at all: exp(-u) = 1 - u phi(u) by the
+        // definition of phi, i.e.  q = T phi(u);  C += q E tau;  T -= q u   (the MUFU pipe runs at a quarter of the FMA rate
+        // and used to bound this loop with one ex2 per update).
+        float C[24], T[24];
 #pragma unroll
-        for (int k = 0; k < 24; ++k) { C[k] = 0.0f; L[k] = 0.0f; }
+        for (int k = 0; k < 24; ++k) { C[k] = 0.0f; T[k] = 1.0f; }
 
         for (int b = 0; b < n_batches; ++b) {
             const int slot = b & 1;
@@ -146,16 +158,28 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                     for (int k = 0; k < 8; ++k) gx[k] = (gx[k] * gy >= thr) ? gx[k] : 0.0f;
                 }
                 const float E[3] = { a0.y, a0.z, a0.w }, A[3] = { a1.x, a1.y, a1.z };
-                if (a1.w < 0.25f) {                         // every u = A tau of this splat is small
+                if (a1.w < 0.03f) {                         // every u = A tau of this splat is tiny: cubic phi
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
                         const float tau = ty * gx[k];
 #pragma unroll
                         for (int ch = 0; ch < 3; ++ch) {
                             const float u = A[ch] * tau;
-                            const float T = ex2_approx(-kLog2e * L[3 * k + ch]);
-                            C[3 * k + ch] = fmaf(T * (E[ch] * tau), phi_small(u), C[3 * k + ch]);
-                            L[3 * k + ch] += u;
+                            const float q = T[3 * k + ch] * phi_tiny(u);
+                            C[3 * k + ch] = fmaf(q, E[ch] * tau, C[3 * k + ch]);
+                            T[3 * k + ch] = fmaf(-q, u, T[3 * k + ch]);
+                        }
+                    }
+                } else if (a1.w < 0.25f) {                  // every u of this splat is small: quintic phi, still no exponential
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const float tau = ty * gx[k];
+#pragma unroll
+                        for (int ch = 0; ch < 3; ++ch) {
+                            const float u = A[ch] * tau;
+                            const float q = T[3 * k + ch] * phi_small(u);
+                            C[3 * k + ch] = fmaf(q, E[ch] * tau, C[3 * k + ch]);
+                            T[3 * k + ch] = fmaf(-q, u, T[3 * k + ch]);
                         }
                     }
                 } else {
@@ -165,11 +189,10 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
 #pragma unroll
                         for (int ch = 0; ch < 3; ++ch) {
                             const float u = A[ch] * tau;
-                            const float T = ex2_approx(-kLog2e * L[3 * k + ch]);
                             const float e = ex2_approx(-kLog2e * u);
                             const float phi = (u < 0.25f) ? phi_small(u) : __fdividef(1.0f - e, u);
-                            C[3 * k + ch] = fmaf(T * (E[ch] * tau), phi, C[3 * k + ch]);
-                            L[3 * k + ch] += u;
+                            C[3 * k + ch] = fmaf(T[3 * k + ch] * (E[ch] * tau), phi, C[3 * k + ch]);
+                            T[3 * k + ch] *= e;
                         }
                     }
                 }
@@ -178,7 +201,7 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
             __syncthreads();
         }
 
-        // partial of this unit: planes C_r, C_g, C_b, L_r, L_g, L_b of 64x64 floats
+        // partial of this unit: planes C_r, C_g, C_b, T_r, T_g, T_b of 64x64 floats
         float *dst = partials + (size_t)unit * (6 * kBlockPx * kBlockPx) + (size_t)ly * kBlockPx + lx;
 #pragma unroll
         for (int ch = 0; ch < 3; ++ch) {
@@ -186,8 +209,8 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
             float4 *pl = reinterpret_cast<float4 *>(dst + (size_t)(3 + ch) * kBlockPx * kBlockPx);
             pc[0] = make_float4(C[ch], C[3 + ch], C[6 + ch], C[9 + ch]);
             pc[1] = make_float4(C[12 + ch], C[15 + ch], C[18 + ch], C[21 + ch]);
-            pl[0] = make_float4(L[ch], L[3 + ch], L[6 + ch], L[9 + ch]);
-            pl[1] = make_float4(L[12 + ch], L[15 + ch], L[18 + ch], L[21 + ch]);
+            pl[0] = make_float4(T[ch], T[3 + ch], T[6 + ch], T[9 + ch]);
+            pl[1] = make_float4(T[12 + ch], T[15 + ch], T[18 + ch], T[21 + ch]);
         }
         __syncthreads();
     }
@@ -205,15 +228,15 @@ merge_absorb_kernel(const float *__restrict__ partials, const uint32_t *__restri
     for (int p = threadIdx.x; p < kBlockPx * kBlockPx; p += blockDim.x) {
         const int X = px0 + (p & (kBlockPx - 1)), Y = py0 + (p >> kBlockShift);
         if (X >= W || Y >= H) continue;
-        float C[3] = { 0.f, 0.f, 0.f }, L[3] = { 0.f, 0.f, 0.f };
+        float C[3] = { 0.f, 0.f, 0.f }, T[3] = { 1.f, 1.f, 1.f };
         for (uint32_t u = u0; u < u1; ++u) {
             const float *src = partials + (size_t)u * (6 * kBlockPx * kBlockPx) + p;
 #pragma unroll
             for (int ch = 0; ch < 3; ++ch) {
                 const float cu = __ldg(src + (size_t)ch * kBlockPx * kBlockPx);
-                const float lu = __ldg(src + (size_t)(3 + ch) * kBlockPx * kBlockPx);
-                C[ch] = fmaf(ex2_approx(-kLog2e * L[ch]), cu, C[ch]);
-                L[ch] += lu;
+                const float tu = __ldg(src + (size_t)(3 + ch) * kBlockPx * kBlockPx);
+                C[ch] = fmaf(T[ch], cu, C[ch]);
+                T[ch] *= tu;
             }
         }
         float *o = out + ((size_t)Y * W + X) * 3;
