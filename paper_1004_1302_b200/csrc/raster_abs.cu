@@ -34,12 +34,27 @@ __device__ __forceinline__ float phi_small(float u)   // (1 - exp(-u)) / u for u
     return fmaf(p, u, 1.0f);
 }
 
-__device__ __forceinline__ float phi_tiny(float u)    // the same for u < 0.03: error < u^4 / 120 < 7e-9
+// one splat with every u = A tau below 0.25 on this lane's 8 pixels: phi of degree kDeg in tau
+template <int kDeg>
+__device__ __forceinline__ void small_u(const float (&tau)[8], const float (&E)[3], const float (&A)[3], float (&C)[24],
+                                        float (&T)[24])
 {
-    float p = -1.0f / 24.0f;
-    p = fmaf(p, u, 1.0f / 6.0f);
-    p = fmaf(p, u, -0.5f);
-    return fmaf(p, u, 1.0f);
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+        const float nA = -A[ch], c1 = 0.5f * nA, c2 = (1.0f / 3.0f) * nA * c1, c3 = 0.25f * nA * c2;
+        const float c4 = 0.2f * nA * c3, c5 = (1.0f / 6.0f) * nA * c4;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            float ph;
+            if (kDeg == 1) ph = fmaf(c1, tau[k], 1.0f);
+            else if (kDeg == 2) ph = fmaf(fmaf(c2, tau[k], c1), tau[k], 1.0f);
+            else if (kDeg == 3) ph = fmaf(fmaf(fmaf(c3, tau[k], c2), tau[k], c1), tau[k], 1.0f);
+            else ph = fmaf(fmaf(fmaf(fmaf(fmaf(c5, tau[k], c4), tau[k], c3), tau[k], c2), tau[k], c1), tau[k], 1.0f);
+            const float z = (T[3 * k + ch] * ph) * tau[k];
+            C[3 * k + ch] = fmaf(z, E[ch], C[3 * k + ch]);
+            T[3 * k + ch] = fmaf(z, nA, T[3 * k + ch]);
+        }
+    }
 }
 
 __global__ void __launch_bounds__(kRasThreads, 1)
@@ -158,30 +173,18 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                     for (int k = 0; k < 8; ++k) gx[k] = (gx[k] * gy >= thr) ? gx[k] : 0.0f;
                 }
                 const float E[3] = { a0.y, a0.z, a0.w }, A[3] = { a1.x, a1.y, a1.z };
-                if (a1.w < 0.03f) {                         // every u = A tau of this splat is tiny: cubic phi
+                if (a1.w < 0.25f) {
+                    // Every u = A tau of this splat is small: no exponential.  phi(A tau) is a polynomial in tau whose
+                    // coefficients c_m = (-A)^m / (m+1)! are per splat and channel;  q = T phi,  z = q tau,  C += z E,  T -= z A.
+                    // The degree follows the bound a1.w on u so that the truncation error of phi stays below 2e-7 (the loop
+                    // is bound by the FMA pipe, every dropped term is a dropped instruction per update).
+                    float tau[8];
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const float tau = ty * gx[k];
-#pragma unroll
-                        for (int ch = 0; ch < 3; ++ch) {
-                            const float u = A[ch] * tau;
-                            const float q = T[3 * k + ch] * phi_tiny(u);
-                            C[3 * k + ch] = fmaf(q, E[ch] * tau, C[3 * k + ch]);
-                            T[3 * k + ch] = fmaf(-q, u, T[3 * k + ch]);
-                        }
-                    }
-                } else if (a1.w < 0.25f) {                  // every u of this splat is small: quintic phi, still no exponential
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const float tau = ty * gx[k];
-#pragma unroll
-                        for (int ch = 0; ch < 3; ++ch) {
-                            const float u = A[ch] * tau;
-                            const float q = T[3 * k + ch] * phi_small(u);
-                            C[3 * k + ch] = fmaf(q, E[ch] * tau, C[3 * k + ch]);
-                            T[3 * k + ch] = fmaf(-q, u, T[3 * k + ch]);
-                        }
-                    }
+                    for (int k = 0; k < 8; ++k) tau[k] = ty * gx[k];
+                    if (a1.w < 1.1e-3f) small_u<1>(tau, E, A, C, T);
+                    else if (a1.w < 0.017f) small_u<2>(tau, E, A, C, T);
+                    else if (a1.w < 0.047f) small_u<3>(tau, E, A, C, T);
+                    else small_u<5>(tau, E, A, C, T);
                 } else {
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
