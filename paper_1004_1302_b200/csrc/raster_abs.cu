@@ -39,18 +39,22 @@ template <int kDeg>
 __device__ __forceinline__ void small_u(const float (&tau)[8], const float (&E)[3], const float (&A)[3], float (&C)[24],
                                         float (&T)[24])
 {
+    float tau2[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) tau2[k] = tau[k] * tau[k];
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) {
         const float nA = -A[ch], c1 = 0.5f * nA, c2 = (1.0f / 3.0f) * nA * c1, c3 = 0.25f * nA * c2;
         const float c4 = 0.2f * nA * c3, c5 = (1.0f / 6.0f) * nA * c4;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            float ph;
-            if (kDeg == 1) ph = fmaf(c1, tau[k], 1.0f);
-            else if (kDeg == 2) ph = fmaf(fmaf(c2, tau[k], c1), tau[k], 1.0f);
-            else if (kDeg == 3) ph = fmaf(fmaf(fmaf(c3, tau[k], c2), tau[k], c1), tau[k], 1.0f);
-            else ph = fmaf(fmaf(fmaf(fmaf(fmaf(c5, tau[k], c4), tau[k], c3), tau[k], c2), tau[k], c1), tau[k], 1.0f);
-            const float z = (T[3 * k + ch] * ph) * tau[k];
+            // s = tau phi(A tau) = tau + tau^2 (c1 + c2 tau + ...):  z = T s,  C += z E,  T -= z A
+            float pl;
+            if (kDeg == 1) pl = c1;
+            else if (kDeg == 2) pl = fmaf(c2, tau[k], c1);
+            else if (kDeg == 3) pl = fmaf(fmaf(c3, tau[k], c2), tau[k], c1);
+            else pl = fmaf(fmaf(fmaf(fmaf(c5, tau[k], c4), tau[k], c3), tau[k], c2), tau[k], c1);
+            const float z = T[3 * k + ch] * fmaf(pl, tau2[k], tau[k]);
             C[3 * k + ch] = fmaf(z, E[ch], C[3 * k + ch]);
             T[3 * k + ch] = fmaf(z, nA, T[3 * k + ch]);
         }
