@@ -36,27 +36,29 @@ __device__ __forceinline__ float phi_small(float u)   // (1 - exp(-u)) / u for u
 
 // one splat with every u = A tau below 0.25 on this lane's 8 pixels: phi of degree kDeg in tau
 template <int kDeg>
-__device__ __forceinline__ void small_u(const float (&tau)[8], const float (&E)[3], const float (&A)[3], float (&C)[24],
-                                        float (&T)[24])
+__device__ __forceinline__ void small_u(const float2 (&tau)[4], const float (&E)[3], const float (&A)[3], float2 (&C)[3][4],
+                                        float2 (&T)[3][4])
 {
-    float tau2[8];
+    float2 tau2[4];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) tau2[k] = tau[k] * tau[k];
+    for (int q = 0; q < 4; ++q) tau2[q] = __fmul2_rn(tau[q], tau[q]);
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) {
         const float nA = -A[ch], c1 = 0.5f * nA, c2 = (1.0f / 3.0f) * nA * c1, c3 = 0.25f * nA * c2;
         const float c4 = 0.2f * nA * c3, c5 = (1.0f / 6.0f) * nA * c4;
+        const float2 nA2 = make_float2(nA, nA), E2 = make_float2(E[ch], E[ch]), k1 = make_float2(c1, c1);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            // s = tau phi(A tau) = tau + tau^2 (c1 + c2 tau + ...):  z = T s,  C += z E,  T -= z A
-            float pl;
-            if (kDeg == 1) pl = c1;
-            else if (kDeg == 2) pl = fmaf(c2, tau[k], c1);
-            else if (kDeg == 3) pl = fmaf(fmaf(c3, tau[k], c2), tau[k], c1);
-            else pl = fmaf(fmaf(fmaf(fmaf(c5, tau[k], c4), tau[k], c3), tau[k], c2), tau[k], c1);
-            const float z = T[3 * k + ch] * fmaf(pl, tau2[k], tau[k]);
-            C[3 * k + ch] = fmaf(z, E[ch], C[3 * k + ch]);
-            T[3 * k + ch] = fmaf(z, nA, T[3 * k + ch]);
+        for (int q = 0; q < 4; ++q) {
+            // s = tau phi(A tau) = tau + tau^2 (c1 + c2 tau + ...):  z = T s,  C += z E,  T -= z A   (two pixels per instruction)
+            float2 pl;
+            if (kDeg == 1) pl = k1;
+            else if (kDeg == 2) pl = __ffma2_rn(make_float2(c2, c2), tau[q], k1);
+            else if (kDeg == 3) pl = __ffma2_rn(__ffma2_rn(make_float2(c3, c3), tau[q], make_float2(c2, c2)), tau[q], k1);
+            else pl = __ffma2_rn(__ffma2_rn(__ffma2_rn(__ffma2_rn(make_float2(c5, c5), tau[q], make_float2(c4, c4)), tau[q],
+                                                       make_float2(c3, c3)), tau[q], make_float2(c2, c2)), tau[q], k1);
+            const float2 z = __fmul2_rn(T[ch][q], __ffma2_rn(pl, tau2[q], tau[q]));
+            C[ch][q] = __ffma2_rn(z, E2, C[ch][q]);
+            T[ch][q] = __ffma2_rn(z, nA2, T[ch][q]);
         }
     }
 }
@@ -151,9 +153,11 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
         // case (every u = A tau of the splat below 0.25) needs no exponential at all: exp(-u) = 1 - u phi(u) by the
         // definition of phi, i.e.  q = T phi(u);  C += q E tau;  T -= q u   (the MUFU pipe runs at a quarter of the FMA rate
         // and used to bound this loop with one ex2 per update).
-        float C[24], T[24];
+        float2 C[3][4], T[3][4];                    // [channel][pixel pair]: two neighbouring pixels share every packed instruction
 #pragma unroll
-        for (int k = 0; k < 24; ++k) { C[k] = 0.0f; T[k] = 1.0f; }
+        for (int ch = 0; ch < 3; ++ch)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { C[ch][q] = make_float2(0.0f, 0.0f); T[ch][q] = make_float2(1.0f, 1.0f); }
 
         for (int b = 0; b < n_batches; ++b) {
             const int slot = b & 1;
@@ -182,9 +186,9 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                     // coefficients c_m = (-A)^m / (m+1)! are per splat and channel;  q = T phi,  z = q tau,  C += z E,  T -= z A.
                     // The degree follows the bound a1.w on u so that the truncation error of phi stays below 2e-7 (the loop
                     // is bound by the FMA pipe, every dropped term is a dropped instruction per update).
-                    float tau[8];
+                    float2 tau[4];
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) tau[k] = ty * gx[k];
+                    for (int q = 0; q < 4; ++q) tau[q] = __fmul2_rn(make_float2(ty, ty), make_float2(gx[2 * q], gx[2 * q + 1]));
                     if (a1.w < 1.1e-3f) small_u<1>(tau, E, A, C, T);
                     else if (a1.w < 0.017f) small_u<2>(tau, E, A, C, T);
                     else if (a1.w < 0.047f) small_u<3>(tau, E, A, C, T);
@@ -195,11 +199,13 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                         const float tau = ty * gx[k];
 #pragma unroll
                         for (int ch = 0; ch < 3; ++ch) {
+                            float &Ck = (k & 1) ? C[ch][k >> 1].y : C[ch][k >> 1].x;
+                            float &Tk = (k & 1) ? T[ch][k >> 1].y : T[ch][k >> 1].x;
                             const float u = A[ch] * tau;
                             const float e = ex2_approx(-kLog2e * u);
                             const float phi = (u < 0.25f) ? phi_small(u) : __fdividef(1.0f - e, u);
-                            C[3 * k + ch] = fmaf(T[3 * k + ch] * (E[ch] * tau), phi, C[3 * k + ch]);
-                            T[3 * k + ch] *= e;
+                            Ck = fmaf(Tk * (E[ch] * tau), phi, Ck);
+                            Tk *= e;
                         }
                     }
                 }
@@ -214,10 +220,10 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
         for (int ch = 0; ch < 3; ++ch) {
             float4 *pc = reinterpret_cast<float4 *>(dst + (size_t)ch * kBlockPx * kBlockPx);
             float4 *pl = reinterpret_cast<float4 *>(dst + (size_t)(3 + ch) * kBlockPx * kBlockPx);
-            pc[0] = make_float4(C[ch], C[3 + ch], C[6 + ch], C[9 + ch]);
-            pc[1] = make_float4(C[12 + ch], C[15 + ch], C[18 + ch], C[21 + ch]);
-            pl[0] = make_float4(T[ch], T[3 + ch], T[6 + ch], T[9 + ch]);
-            pl[1] = make_float4(T[12 + ch], T[15 + ch], T[18 + ch], T[21 + ch]);
+            pc[0] = make_float4(C[ch][0].x, C[ch][0].y, C[ch][1].x, C[ch][1].y);
+            pc[1] = make_float4(C[ch][2].x, C[ch][2].y, C[ch][3].x, C[ch][3].y);
+            pl[0] = make_float4(T[ch][0].x, T[ch][0].y, T[ch][1].x, T[ch][1].y);
+            pl[1] = make_float4(T[ch][2].x, T[ch][2].y, T[ch][3].x, T[ch][3].y);
         }
         __syncthreads();
     }
