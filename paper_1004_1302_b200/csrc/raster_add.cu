@@ -261,12 +261,17 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
             gather(b + 2, slot);                 // rec[slot] held batch b, already turned into factors
             produce(b + 1, slot ^ 1);
             const unsigned cA = sm.cls[slot][lane][tA], cB = sm.cls[slot][lane][tB];
-            unsigned m;
-            m = __ballot_sync(0xffffffffu, cA == 2);
-            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
-            m = __ballot_sync(0xffffffffu, cB == 2);
-            while (m) { const int s = __ffs(m) - 1; m &= m - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
-            // rim tiles: the items of the two tiles are walked in pairs, two independent chains per iteration
+            // inside tiles, then rim tiles: the items of the two tiles are walked in pairs, two independent chains per iteration
+            unsigned iA = __ballot_sync(0xffffffffu, cA == 2), iB = __ballot_sync(0xffffffffu, cB == 2);
+            while (iA && iB) {
+                const int sA = __ffs(iA) - 1, sB = __ffs(iB) - 1;
+                iA &= iA - 1;
+                iB &= iB - 1;
+                splat_tile<false>(sm.gx[slot][sA], sm.row[slot][sA], xA, yA, accA);
+                splat_tile<false>(sm.gx[slot][sB], sm.row[slot][sB], xB, yB, accB);
+            }
+            while (iA) { const int s = __ffs(iA) - 1; iA &= iA - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xA, yA, accA); }
+            while (iB) { const int s = __ffs(iB) - 1; iB &= iB - 1; splat_tile<false>(sm.gx[slot][s], sm.row[slot][s], xB, yB, accB); }
             unsigned mA = __ballot_sync(0xffffffffu, cA == 1), mB = __ballot_sync(0xffffffffu, cB == 1);
             while (mA && mB) {
                 const int sA = __ffs(mA) - 1, sB = __ffs(mB) - 1;
