@@ -106,7 +106,7 @@ __device__ __forceinline__ void count_bins(uint32_t bins, uint32_t *hist, int nb
 }
 
 template <bool kAbsorb>
-__global__ void __launch_bounds__(kProjThreads)
+__global__ void __launch_bounds__(kProjThreads, 4)
 project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, const float *__restrict__ lutE,
                const float *__restrict__ lutA, void *__restrict__ records, uint32_t *__restrict__ bin_count,
                uint32_t *__restrict__ zkeys, WorkHead *head, DebugProjectOut dbg, int has_dbg, int vec_ok,
