@@ -31,7 +31,10 @@
  * line integral, the closed-form flux of a splat, energy conservation, permutation
  * invariance, brute-force RK4 integration of Eq. (1) on tiny inputs, absorb == additive when
  * A == E, front-to-back == back-to-front, camera conventions, scale invariance, LUT nodes,
- * tie order.  Conventions the paper leaves open (f = 3 default, rho_0 = I, z_near, fov axis,
+ * tie order; P17 per-type table offset and per-type brightness / abs_brightness (two types
+ * with different tables, expected values written by hand from the inputs); P18 the region-of-
+ * interest path (off-origin ROI == hand-evaluated single-splat closed form at the ROI's pixel
+ * centres, and == the crop of the full frame bit for bit, both modes).  Conventions the paper leaves open (f = 3 default, rho_0 = I, z_near, fov axis,
  * image orientation, slab reading under overlap) are "parity unpinned" by the paper: they
  * are pinned only by DESIGN.md.
  */

@@ -457,3 +457,132 @@ def test_p16_vector_colouring_reduces_to_the_scalar_path():
     wa = mk(pts, c, lut_e=const_lut(), lut_a=const_lut(), brightness=(1.3,), abs_brightness=(1.3,), mode=ABSORB)
     wa.vec = vec
     np.testing.assert_allclose(oracle.render_vector(wa), oracle.render_vector(wv.__class__(**{**wv.__dict__, "vec": vec})), rtol=1e-9, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# P17: per-type colour tables and per-type brightness (PAPER.md:75 transfer function per particle
+# property; readings R7, R14).  Two types with DIFFERENT tables and DIFFERENT brightness /
+# abs_brightness.  Expected values are written by hand from the input tables: a particle at table
+# node k of type t has E = brightness[t] * tabE[t][k], A = abs_brightness[t] * tabA[t][k], and its
+# image is the single-splat closed form of O6 / O8 evaluated here, not by the oracle.
+# ------------------------------------------------------------------------------------------------
+_T2E = np.array([[[0.10, 0.20, 0.30], [0.50, 0.10, 0.90], [0.00, 1.00, 0.40]],
+                 [[0.80, 0.60, 0.05], [0.25, 0.75, 0.35], [0.90, 0.15, 0.65]]], np.float32)
+_T2A = np.array([[[1.50, 0.10, 0.60], [0.05, 0.90, 2.00], [0.70, 0.30, 0.20]],
+                 [[0.40, 1.20, 0.15], [2.50, 0.45, 0.85], [0.12, 0.55, 1.75]]], np.float32)
+_BR2, _AB2 = (1.25, 0.375), (0.5, 3.0)            # exact in binary32
+
+
+def test_p17_per_type_tables_and_brightness_in_the_splat_table():
+    c = cam(w=16, h=16)
+    pts, types = [], []
+    for t in (0, 1):
+        for cv in (0.0, 0.5, 1.0, 0.25):          # three nodes and one midpoint
+            pts.append((0, 0, 0, 0.1, 1, cv))
+            types.append(t)
+    w = mk(pts, c, lut_e=_T2E, lut_a=_T2A, brightness=_BR2, abs_brightness=_AB2, mode=ABSORB, types=types)
+    tab, ok = oracle.splat_table(w)
+    assert ok.all()
+    LE, LA = _T2E.astype(np.float64), _T2A.astype(np.float64)
+    row = 0
+    for t in (0, 1):
+        for k in range(3):
+            np.testing.assert_array_equal(tab[row, 5:8], _BR2[t] * LE[t, k])
+            np.testing.assert_array_equal(tab[row, 8:11], _AB2[t] * LA[t, k])
+            row += 1
+        np.testing.assert_allclose(tab[row, 5:8], _BR2[t] * 0.5 * (LE[t, 0] + LE[t, 1]), rtol=1e-15)
+        np.testing.assert_allclose(tab[row, 8:11], _AB2[t] * 0.5 * (LA[t, 0] + LA[t, 1]), rtol=1e-15)
+        row += 1
+    # additive mode: A == E of the particle's own type and brightness
+    tab0, _ = oracle.splat_table(w, mode=ADDITIVE)
+    np.testing.assert_array_equal(tab0[:, 8:11], tab0[:, 5:8])
+    np.testing.assert_array_equal(tab0[:, 5:8], tab[:, 5:8])
+
+
+@pytest.mark.parametrize("mode", [ADDITIVE, ABSORB])
+def test_p17_per_type_single_splat_image_closed_form(mode):
+    """One particle per type, far apart on the screen, each at a table node of its own type: every pixel
+    equals the hand-evaluated single-splat value with that type's table row and brightness."""
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=96, h=48)
+    F = 48.0 / np.tan(np.deg2rad(10.0))
+    #            x     y    z    r     I    colval            type, node
+    pts = [(-1.0, 0.1, 0.0, 0.15, 0.8, 0.5), (1.1, -0.2, 0.5, 0.12, 1.5, 1.0)]
+    types, nodes = [1, 0], [1, 2]
+    w = mk(pts, c, lut_e=_T2E, lut_a=_T2A, brightness=_BR2, abs_brightness=_AB2, mode=mode, types=types)
+    img = oracle.render(w, raw=True)
+    jj, ii = np.meshgrid(np.arange(c.height) + 0.5, np.arange(c.width) + 0.5, indexing="ij")
+    expect = np.zeros((c.height, c.width, 3))
+    for p in range(2):
+        x, y, z, r, I = (float(np.float32(v)) for v in pts[p][:5])
+        zc = z + 10.0                              # right = fwd x up = (-1, 0, 0) for this camera (R2)
+        sx, sy, sg = c.width / 2 - F * x / zc, c.height / 2 - F * y / zc, F * r / zc
+        d2 = (ii - sx) ** 2 + (jj - sy) ** 2
+        tau = np.where(d2 <= (3.0 * sg) ** 2, I * r * SQRT_PI * np.exp(-d2 / sg ** 2), 0.0)[:, :, None]
+        E = _BR2[types[p]] * _T2E[types[p], nodes[p]].astype(np.float64)
+        if mode == ADDITIVE:
+            expect += E * tau
+        else:
+            A = _AB2[types[p]] * _T2A[types[p], nodes[p]].astype(np.float64)
+            u = A * tau
+            expect += E * tau * np.where(u > 0, -np.expm1(-u) / np.where(u > 0, u, 1.0), 1.0)   # discs do not overlap
+    assert (expect[:, :48] > 0).any() and (expect[:, 48:] > 0).any() and np.all(expect[:, 46:50] == 0)   # disjoint discs
+    np.testing.assert_allclose(img, expect, rtol=1e-11, atol=1e-15)
+
+
+def test_p17_type_out_of_range_is_culled_and_in_range_types_differ():
+    """R6: type >= n_types contributes exactly 0; the same particle rendered as type 0 and as type 1 differs by the
+    hand-computed ratio of brightness * table entry (a `type -> 0` slip anywhere would make them equal)."""
+    c = cam(w=16, h=16)
+    lut = np.stack([const_lut((1.0, 0.5, 0.25))[0], const_lut((0.5, 1.0, 0.125))[0]])
+    kw = dict(lut_e=lut, brightness=(1.0, 2.0))
+    S0 = oracle.render(mk([(0, 0, 0, 0.2, 1, 0)], c, types=[0], **kw), raw=True)
+    S1 = oracle.render(mk([(0, 0, 0, 0.2, 1, 0)], c, types=[1], **kw), raw=True)
+    S3 = oracle.render(mk([(0, 0, 0, 0.2, 1, 0)], c, types=[3], **kw), raw=True)
+    assert S0.max() > 0 and np.all(S3 == 0.0)
+    np.testing.assert_allclose(S1[..., 0], S0[..., 0] * 1.0, rtol=1e-15)      # 2.0 * 0.5  vs 1.0 * 1.0
+    np.testing.assert_allclose(S1[..., 1], S0[..., 1] * 4.0, rtol=1e-15)      # 2.0 * 1.0  vs 1.0 * 0.5
+    np.testing.assert_allclose(S1[..., 2], S0[..., 2] * 1.0, rtol=1e-15)      # 2.0 * .125 vs 1.0 * 0.25
+
+
+# ------------------------------------------------------------------------------------------------
+# P18: the region-of-interest path of the oracle (SURVEY.md 8(c) "Oracle practicalities"): the only
+# checker of the full-size images.  An off-origin, non-aligned ROI must equal (a) the hand-evaluated
+# single-splat closed form a exp(-d^2/sigma_s^2) at the ROI's own pixel centres, (b) the same crop of
+# the full-frame render bit for bit, in both modes, with many overlapping particles (the per-pixel
+# visiting order is the same, so even the rounding is).
+# ------------------------------------------------------------------------------------------------
+def test_p18_roi_single_splat_closed_form_at_roi_pixels():
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=80, h=64)
+    F = 40.0 / np.tan(np.deg2rad(10.0))
+    x, y, z, r, I = (float(np.float32(v)) for v in (0.31, -0.17, 0.4, 0.21, 0.9))
+    w = mk([(x, y, z, r, I, 0.0)], c, lut_e=const_lut((0.9, 0.6, 0.3)))
+    zc = z + 10.0
+    sx, sy, sg = 40.0 - F * x / zc, 32.0 - F * y / zc, F * r / zc      # right = fwd x up = (-1, 0, 0) (R2)
+    a = np.array([0.9, 0.6, 0.3], np.float32).astype(np.float64) * I * r * SQRT_PI
+    for roi in [(14, 21, 43, 50), (33, 33, 34, 34), (0, 33, 80, 40), (29, 0, 36, 64), (60, 5, 77, 11)]:
+        x0, y0, x1, y1 = roi
+        got = oracle.render(w, roi=roi, raw=True)
+        assert got.shape == (y1 - y0, x1 - x0, 3)
+        jj, ii = np.meshgrid(np.arange(y0, y1) + 0.5, np.arange(x0, x1) + 0.5, indexing="ij")
+        d2 = (ii - sx) ** 2 + (jj - sy) ** 2
+        expect = np.where(d2 <= (3.0 * sg) ** 2, np.exp(-d2 / sg ** 2), 0.0)[:, :, None] * a
+        np.testing.assert_allclose(got, expect, rtol=1e-11, atol=1e-300)
+    assert oracle.render(w, roi=(14, 21, 43, 50), raw=True).max() > 0.05
+
+
+@pytest.mark.parametrize("mode", [ADDITIVE, ABSORB])
+def test_p18_roi_equals_crop_of_full_frame(mode):
+    rs = np.random.RandomState(23)
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=150, h=131)
+    n = 600
+    pts = np.stack([rs.uniform(-2.2, 2.2, n), rs.uniform(-2.0, 2.0, n), rs.uniform(-1, 1, n),
+                    np.exp(rs.uniform(np.log(0.01), np.log(0.6), n)), rs.uniform(0.5, 1.5, n), rs.uniform(0, 1, n)], 1)
+    types = rs.randint(0, 2, n)
+    w = mk(pts, c, lut_e=_T2E, lut_a=_T2A, brightness=_BR2, abs_brightness=_AB2, mode=mode, types=types)
+    full = oracle.render(w)
+    assert full.max() > 0.1
+    for roi in [(37, 21, 101, 85), (1, 1, 150, 131), (149, 130, 150, 131), (64, 64, 128, 128), (13, 90, 77, 107),
+                (100, 0, 150, 3)]:
+        x0, y0, x1, y1 = roi
+        got = oracle.render(w, roi=roi)
+        np.testing.assert_array_equal(got, full[y0:y1, x0:x1])
