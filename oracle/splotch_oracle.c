@@ -310,6 +310,8 @@ int orc_splat_table(int64_t n, const float *x, const float *y, const float *z, c
  *       constant, Eq. (1) integrates to
  *           I_c <- I_c exp(-u_c) + E_pc tau_p phi(u_c),  u_c = A_pc tau_p,
  *           phi(u) = (1 - exp(-u)) / u, phi(0) = 1            (slab reading R10, R15)
+ *       The slab solution of Eq. (1) holds for either sign of u; negative I, E or A are
+ *       unphysical but "used as given" (reading R20), so phi is evaluated for u < 0 as well.
  *
  * `seq[0..m)` lists the particles to visit: index order (additive) or depth order nearest
  * first (absorb; visited backwards).  Rows are split into bands over the OpenMP threads;
@@ -344,7 +346,7 @@ static void render_rows(const double *table, const int64_t *seq, int64_t m, int3
                 } else {
                     for (int c = 0; c < 3; ++c) {
                         double u = t[8 + c] * tau;
-                        double phi = (u > 0.0) ? (-expm1(-u) / u) : 1.0;
+                        double phi = (u != 0.0) ? (-expm1(-u) / u) : 1.0;   /* either sign of u: reading R20 */
                         px[c] = px[c] * exp(-u) + t[5 + c] * tau * phi;
                     }
                 }

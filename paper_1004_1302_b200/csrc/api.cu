@@ -4,13 +4,15 @@
 #include <math.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "../../include/splotch.h"
 #include "common.cuh"
 
 namespace splotch {
 
 thread_local int g_last_cuda_error = 0;
-unsigned long long g_launch_count = 0;
+std::atomic<unsigned long long> g_launch_count{0};
 
 // ---------------------------------------------------------------------------------------------
 // optional per-stage timing of splotch_render with CUDA events on the caller's stream
@@ -24,9 +26,11 @@ struct Profile {
     cudaEvent_t ev[kMaxProfiledCalls][kStages + 1];
     bool created[kMaxProfiledCalls] = {};
 } g_prof;
+std::mutex g_prof_mutex;            // the profile is one per process: calls from several threads are serialised
 
 void prof_mark(int stage, cudaStream_t st)
 {
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     if (!g_prof.on || g_prof.calls >= kMaxProfiledCalls) return;
     const int c = g_prof.calls;
     if (!g_prof.created[c]) {
@@ -39,18 +43,23 @@ void prof_mark(int stage, cudaStream_t st)
 }
 }  // namespace
 
+int current_device()
+{
+    int dev = 0;
+    return cudaGetDevice(&dev) == cudaSuccess ? dev : 0;
+}
+
 int sm_count()
 {
-    static int cached = 0;
-    if (cached == 0) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            cached = n;
-        else
-            return 148;
+    static std::atomic<int> cached[kMaxDevices];
+    const int dev = current_device();
+    const bool slot = dev >= 0 && dev < kMaxDevices;
+    int n = slot ? cached[dev].load(std::memory_order_relaxed) : 0;
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+        if (slot) cached[dev].store(n, std::memory_order_relaxed);
     }
-    return cached;
+    return n;
 }
 
 namespace {
@@ -262,7 +271,7 @@ int run_lists(const Ctx &c, int64_t n, uint64_t max_pairs, uint32_t **list_out)
     if (rc) return rc;
     bool in_tmp = false;
     rc = launch_sort_pairs(c.at<uint32_t>(c.L.zkeys), c.at<uint32_t>(c.L.ids), c.at<uint32_t>(c.L.zkeys_tmp),
-                           c.at<uint32_t>(c.L.ids_tmp), n, nullptr, 32, c.ws + c.L.sort_scratch, c.st, &in_tmp);
+                           c.at<uint32_t>(c.L.ids_tmp), n, nullptr, 32, c.ws + c.L.sort_scratch, c.st, &in_tmp, &c.head()->status);
     if (rc) return rc;
     const uint32_t *sorted = in_tmp ? c.at<uint32_t>(c.L.ids_tmp) : c.at<uint32_t>(c.L.ids);
     rc = launch_pair_counts(c.ws + c.L.records, rec_bytes, sorted, n, c.at<uint32_t>(c.L.pair_count), c.st);
@@ -275,7 +284,7 @@ int run_lists(const Ctx &c, int64_t n, uint64_t max_pairs, uint32_t **list_out)
     // stable split by bin keeps the depth order inside every bin; the pair count lives on the device
     rc = launch_sort_pairs(c.at<uint32_t>(c.L.pair_bin), c.at<uint32_t>(c.L.pair_id), c.at<uint32_t>(c.L.pair_bin_tmp),
                            c.at<uint32_t>(c.L.list), (int64_t)max_pairs, &c.head()->pairs, bits_for(c.n_bins),
-                           c.ws + c.L.sort_scratch, c.st, &in_tmp);
+                           c.ws + c.L.sort_scratch, c.st, &in_tmp, &c.head()->status);
     if (rc) return rc;
     *list_out = in_tmp ? c.at<uint32_t>(c.L.list) : c.at<uint32_t>(c.L.pair_id);
     return SPLOTCH_OK;
@@ -402,6 +411,7 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
 
 int splotch_profile_enable(int on)
 {
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     g_prof.on = on != 0;
     g_prof.calls = 0;
     return SPLOTCH_OK;
@@ -410,6 +420,7 @@ int splotch_profile_enable(int on)
 int splotch_profile_read(double *stage_ms, int64_t *calls)
 {
     if (!stage_ms) return SPLOTCH_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_prof_mutex);
     for (int k = 0; k < kStages; ++k) stage_ms[k] = 0.0;
     const int n = g_prof.calls;
     if (calls) *calls = n;
@@ -424,7 +435,7 @@ int splotch_profile_read(double *stage_ms, int64_t *calls)
     return SPLOTCH_OK;
 }
 
-unsigned long long splotch_launch_count(void) { return g_launch_count; }
+unsigned long long splotch_launch_count(void) { return g_launch_count.load(std::memory_order_relaxed); }
 
 int splotch_workspace_status(const void *workspace, void *stream, int32_t *status, uint64_t *visible, uint64_t *pairs)
 {

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace splotch {
 
 // ---------------------------------------------------------------------------------------------
@@ -102,15 +104,34 @@ extern thread_local int g_last_cuda_error;
         }                                                        \
     } while (0)
 
-extern unsigned long long g_launch_count;   // kernels this library has launched (bench.py "gpu_launches")
-#define SPLOTCH_LAUNCH_CHECK()                      \
-    do {                                            \
-        ++::splotch::g_launch_count;                \
-        SPLOTCH_CUDA_TRY(cudaGetLastError());       \
+extern std::atomic<unsigned long long> g_launch_count;   // kernels this library has launched (bench.py "gpu_launches")
+#define SPLOTCH_LAUNCH_CHECK()                                                      \
+    do {                                                                            \
+        ::splotch::g_launch_count.fetch_add(1ull, std::memory_order_relaxed);       \
+        SPLOTCH_CUDA_TRY(cudaGetLastError());                                       \
     } while (0)
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
-int sm_count();
+
+// Per-DEVICE state (function attributes and the SM count belong to a device, not to the process): caches are keyed by
+// the ordinal of the calling thread's current device, so one process may render on several GPUs.
+constexpr int kMaxDevices = 64;
+int current_device();                                   // ordinal of the current device, 0 if it cannot be read
+int sm_count();                                         // SMs of the current device
+
+// opt a kernel in to `bytes` of dynamic shared memory once per device
+struct SmemOptIn {
+    std::atomic<unsigned char> done[kMaxDevices];
+};
+template <typename Kernel>
+inline int smem_opt_in(SmemOptIn &state, Kernel kernel, int bytes)
+{
+    const int dev = current_device();
+    if (dev >= 0 && dev < kMaxDevices && state.done[dev].load(std::memory_order_acquire)) return 0;
+    SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    if (dev >= 0 && dev < kMaxDevices) state.done[dev].store(1, std::memory_order_release);
+    return 0;
+}
 
 // ---------------------------------------------------------------------------------------------
 // launchers (each only enqueues on `st`)
@@ -137,7 +158,7 @@ int launch_scan_u32_u32(const uint32_t *in, uint32_t *out, int64_t n, void *scra
 uint64_t sort_scratch_bytes(int64_t n);
 int launch_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
                       const unsigned long long *n_dev, int key_bits, void *scratch, cudaStream_t st,
-                      bool *result_in_tmp);
+                      bool *result_in_tmp, const int32_t *status_dev = nullptr);
 
 // project.cu (K1): records + fused bin counts (+ optional debug outputs, + depth keys in absorb mode)
 int launch_project(const ParticlePtrs &p, int64_t n, const CameraConst &cam, const RenderConst &rc,

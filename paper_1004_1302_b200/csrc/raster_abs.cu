@@ -16,7 +16,7 @@ constexpr int kRasThreads = 512;
 struct SmemAbs {
     float fac[2][kBatch][128];
     float4 amp0[2][kBatch];             // tau0, E_r, E_g, E_b
-    float4 amp1[2][kBatch];             // A_r, A_g, A_b, max(A) * tau0
+    float4 amp1[2][kBatch];             // A_r, A_g, A_b, max|A| * |tau0|
     unsigned char cls[2][kBatch][16];
     SplatAbs rec[2][kBatch];
     uint32_t ids[kChunkAbs];
@@ -138,7 +138,9 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                 const float4 r1 = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 1);   // tau0, E
                 const float4 r2 = *(reinterpret_cast<const float4 *>(&sm.rec[slot][s]) + 2);   // A, bins
                 sm.amp0[slot][s] = r1;
-                sm.amp1[slot][s] = make_float4(r2.x, r2.y, r2.z, fmaxf(fmaxf(r2.x, r2.y), r2.z) * r1.x);
+                // bound on |u| = |A tau| over the splat: absolute values, so that negative (unphysical, but accepted: reading
+                // R20) A or I never select a polynomial tier whose truncation bound does not hold
+                sm.amp1[slot][s] = make_float4(r2.x, r2.y, r2.z, fmaxf(fmaxf(fabsf(r2.x), fabsf(r2.y)), fabsf(r2.z)) * fabsf(r1.x));
             }
         };
 
@@ -203,7 +205,7 @@ raster_absorb_kernel(const SplatAbs *__restrict__ records, const uint32_t *__res
                             float &Tk = (k & 1) ? T[ch][k >> 1].y : T[ch][k >> 1].x;
                             const float u = A[ch] * tau;
                             const float e = ex2_approx(-kLog2e * u);
-                            const float phi = (u < 0.25f) ? phi_small(u) : __fdividef(1.0f - e, u);
+                            const float phi = (fabsf(u) < 0.25f) ? phi_small(u) : __fdividef(1.0f - e, u);
                             Ck = fmaf(Tk * (E[ch] * tau), phi, Ck);
                             Tk *= e;
                         }
@@ -263,12 +265,8 @@ int launch_raster_absorb(const SplatAbs *records, const uint32_t *list, const ui
                          const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *partials,
                          WorkHead *head, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_absorb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SmemAbs)));
-        attr_set = true;
-    }
+    static SmemOptIn opt;
+    if (int rc = smem_opt_in(opt, raster_absorb_kernel, (int)sizeof(SmemAbs))) return rc;
     raster_absorb_kernel<<<sm_count(), kRasThreads, sizeof(SmemAbs), st>>>(records, list, bin_offset, unit_prefix,
                                                                            rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr,
                                                                            partials, head);

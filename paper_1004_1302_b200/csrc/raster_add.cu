@@ -341,14 +341,9 @@ int launch_raster_additive(const SplatAdd *records, const uint32_t *list, const 
                            const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
                            WorkHead *head, int tensor, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SmemAdd)));
-        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SmemAdd)));
-        attr_set = true;
-    }
+    static SmemOptIn opt_mma, opt_alu;
+    if (int rc = smem_opt_in(opt_mma, raster_additive_kernel<true>, (int)sizeof(SmemAdd))) return rc;
+    if (int rc = smem_opt_in(opt_alu, raster_additive_kernel<false>, (int)sizeof(SmemAdd))) return rc;
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
     if (tensor != 0) {
         raster_additive_kernel<true><<<sm_count() * 2, kRasThreads, sizeof(SmemAdd), st>>>(

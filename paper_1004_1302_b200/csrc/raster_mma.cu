@@ -518,12 +518,8 @@ int launch_raster_additive_mma(const SplatAdd *records, uint32_t *list, const ui
                                const uint32_t *unit_prefix, const RenderConst &rc, const CameraConst &cam, float *S,
                                WorkHead *head, int tensor, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPLOTCH_CUDA_TRY(cudaFuncSetAttribute(raster_additive_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SmemMma)));
-        attr_set = true;
-    }
+    static SmemOptIn opt;
+    if (int rc = smem_opt_in(opt, raster_additive_mma_kernel, (int)sizeof(SmemMma))) return rc;
     const int vec_ok = (cam.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15u) == 0);
     raster_additive_mma_kernel<<<sm_count() * 2, kMmaThreads, sizeof(SmemMma), st>>>(
         records, list, bin_offset, unit_prefix, rc.nbx * rc.nby, rc.nbx, cam.W, cam.H, rc.thr, S, head, vec_ok, tensor);

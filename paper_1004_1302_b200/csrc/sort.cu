@@ -20,10 +20,11 @@ constexpr int kRadix = 256;
 
 __global__ void __launch_bounds__(kSortThreads)
 sort_hist_kernel(const uint32_t *__restrict__ keys, long long n_cap, const unsigned long long *__restrict__ n_dev,
-                 int shift, uint32_t *__restrict__ hist, long long n_tiles)
+                 int shift, uint32_t *__restrict__ hist, long long n_tiles, const int32_t *__restrict__ status)
 {
     __shared__ uint32_t s_hist[kRadix];
-    const long long n = n_dev ? min((long long)*n_dev, n_cap) : n_cap;   // item count may live on the device
+    // item count may live on the device; a failed render (status != 0: pair capacity exceeded) sorts nothing
+    const long long n = (status && *status != 0) ? 0 : n_dev ? min((long long)*n_dev, n_cap) : n_cap;
     const long long tile = blockIdx.x;
     if (threadIdx.x < kRadix) s_hist[threadIdx.x] = 0u;
     __syncthreads();
@@ -41,11 +42,12 @@ __global__ void __launch_bounds__(kSortThreads)
 sort_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                     uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out, long long n_cap,
                     const unsigned long long *__restrict__ n_dev, int shift,
-                    const uint32_t *__restrict__ hist_scanned, long long n_tiles, int write_keys)
+                    const uint32_t *__restrict__ hist_scanned, long long n_tiles, int write_keys,
+                    const int32_t *__restrict__ status)
 {
     __shared__ uint32_t s_wcnt[kSortWarps][kRadix];
     __shared__ uint32_t s_gbase[kRadix];
-    const long long n = n_dev ? min((long long)*n_dev, n_cap) : n_cap;
+    const long long n = (status && *status != 0) ? 0 : n_dev ? min((long long)*n_dev, n_cap) : n_cap;
     const long long tile = blockIdx.x;
     if (tile * kSortTile >= n) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -106,9 +108,11 @@ uint64_t sort_scratch_bytes(int64_t n)
 
 // Sorts on key bits [0, key_bits).  Ping-pongs between (keys, vals) and (keys_tmp, vals_tmp);
 // *result_in_tmp tells where the result ended.  `n` is the capacity the grids are sized for; when
-// n_dev != NULL the actual item count min(*n_dev, n) is read on the device (no host sync).
+// n_dev != NULL the actual item count min(*n_dev, n) is read on the device (no host sync); when status_dev != NULL and
+// *status_dev != 0 (a render that already failed) every pass returns at once.
 int launch_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
-                      const unsigned long long *n_dev, int key_bits, void *scratch, cudaStream_t st, bool *result_in_tmp)
+                      const unsigned long long *n_dev, int key_bits, void *scratch, cudaStream_t st, bool *result_in_tmp,
+                      const int32_t *status_dev)
 {
     *result_in_tmp = false;
     if (n <= 0 || key_bits <= 0) return 0;
@@ -123,12 +127,12 @@ int launch_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32
     uint32_t *ki = keys, *vi = vals, *ko = keys_tmp, *vo = vals_tmp;
     for (int p = 0; p < passes; ++p) {
         const int shift = p * 8;
-        sort_hist_kernel<<<(unsigned)n_tiles, kSortThreads, 0, st>>>(ki, (long long)n, n_dev, shift, hist, n_tiles);
+        sort_hist_kernel<<<(unsigned)n_tiles, kSortThreads, 0, st>>>(ki, (long long)n, n_dev, shift, hist, n_tiles, status_dev);
         SPLOTCH_LAUNCH_CHECK();
         int rc = launch_scan_u32_u32(hist, hist_scanned, m, scan_scratch, st);
         if (rc) return rc;
         sort_scatter_kernel<<<(unsigned)n_tiles, kSortThreads, 0, st>>>(ki, vi, ko, vo, (long long)n, n_dev, shift,
-                                                                        hist_scanned, n_tiles, 1);
+                                                                        hist_scanned, n_tiles, 1, status_dev);
         SPLOTCH_LAUNCH_CHECK();
         uint32_t *t = ki; ki = ko; ko = t;
         t = vi; vi = vo; vo = t;

@@ -36,6 +36,9 @@ def shard_workload(w, world: int, rank: int):
     for k in ("x", "y", "z", "r", "I", "colval"):
         setattr(sh, k, getattr(w, k)[s:e])
     sh.type = None if w.type is None else w.type[s:e]
+    vec = getattr(w, "vec", None)           # optional (n, 3) vector colouring follows its particles
+    if vec is not None:
+        sh.vec = vec[s:e]
     sh.n = e - s
     return sh
 

@@ -339,6 +339,53 @@ def test_edge_cases(B):
     assert float(sc.render().abs().max()) > 0.0
 
 
+@pytest.mark.parametrize("mode", [ADDITIVE, ABSORB])
+def test_pair_capacity_contract_both_modes(B, mode):
+    """D > max_pairs (and max_pairs = 0): SPLOTCH_ERR_WORKSPACE in the status head, a ZERO image, never a partial one;
+    the same workspace then serves a correctly sized render (the absorb failure path had never run)."""
+    w = workloads.make("C4" if mode == ABSORB else "C2", 30_000, width=300, height=200)
+    sc = _scene(w)
+    pairs, vis = sc.count_pairs()
+    assert pairs > vis > 1000
+    good = None
+    for cap in (pairs, pairs // 3, 0, pairs):
+        sc.reserve(max_pairs=max(cap, pairs))       # the allocation is large enough; only the declared capacity varies
+        sc.max_pairs = cap
+        img = torch.full((200, 300, 3), 7.0, dtype=torch.float32, device="cuda")
+        sc.render(out=img, check=False)
+        status, v2, p2 = B.splotch_workspace_status(sc._aligned(sc.workspace))
+        assert p2 == pairs and v2 == vis
+        if cap >= pairs:
+            assert status == B.SPLOTCH_OK and float(img.max()) > 0.0 and float(img.max()) < 7.0
+            if good is None:
+                good = img.cpu().numpy()
+            else:
+                np.testing.assert_allclose(img.cpu().numpy(), good, rtol=2e-5, atol=1e-6)
+        else:
+            assert status == B.SPLOTCH_ERR_WORKSPACE
+            assert float(img.abs().max()) == 0.0
+
+
+def test_negative_coefficients_follow_the_oracle(B):
+    """Reading R20: negative I, E, A are used as given (the slab solution of Eq. (1) holds for either sign of u); the
+    absorb kernel must pick its polynomial tier from |A tau|."""
+    rs = np.random.RandomState(9)
+    c = cam(eye=(0, 0, -10.0), fov=20.0, w=160, h=96)
+    n = 500
+    pts = np.stack([rs.uniform(-1.6, 1.6, n), rs.uniform(-1.0, 1.0, n), rs.uniform(-2, 2, n),
+                    rs.uniform(0.05, 0.5, n), rs.uniform(-2.0, 3.0, n), rs.uniform(0, 1, n)], 1)
+    lut_e = np.array([[0.2, -0.5, 0.9], [1.0, 0.3, -0.1]], np.float32)
+    lut_a = np.array([[-1.5, 0.1, 0.6], [0.5, -0.9, 2.0]], np.float32)
+    w = mk(pts, c, lut_e=lut_e, lut_a=lut_a, mode=ABSORB, support_f=3.2, abs_brightness=(0.2,))
+    out, ref = _render_both(w)
+    assert ref.max() > 0.3 and ref.min() < -0.05
+    _tol_check_masked(w, out, ref)
+    for tensor in (True, False):
+        out, ref = _render_both(w, raw=True, mode=ADDITIVE, tensor=tensor)
+        assert ref.min() < -0.05
+        _tol_check_masked(w, out, ref)
+
+
 def test_repeat_calls_and_orbit_cameras(B):
     """C5's use case: several cameras over one resident particle set; same camera twice gives the same image."""
     w = workloads.make("C5", 300_000, width=256, height=256)

@@ -38,6 +38,15 @@ def test_shard_workload_slices_every_array():
     assert parts[0].brightness == w.brightness and parts[0].cameras is w.cameras
 
 
+def test_shard_workload_slices_the_colour_vectors():
+    """vector colouring (f3) + particle sharding (e): every rank must see ITS particles' vectors."""
+    w = workloads.make("C1", 1001)
+    w.vec = np.random.RandomState(0).uniform(0, 1, (w.n, 3)).astype(np.float32)
+    parts = [multi.shard_workload(w, 3, r) for r in range(3)]
+    np.testing.assert_array_equal(np.concatenate([p.vec for p in parts]), w.vec)
+    assert [len(p.vec) for p in parts] == [334, 334, 333] and w.vec.shape == (1001, 3)
+
+
 def _free_port():
     s = socket.socket()
     s.bind(("127.0.0.1", 0))
@@ -46,15 +55,18 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, q):
+def _worker(rank, world, port, q, vec=False):
     import torch.distributed as dist
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         w = workloads.make("C1", 20_000, width=96, height=64)
+        if vec:
+            w.vec = np.random.RandomState(5).uniform(0, 1, (w.n, 3)).astype(np.float32)
         sh = multi.shard_workload(w, world, rank)
-        partial = torch.from_numpy(oracle.render(sh, raw=True))          # this rank's raw S (double)
+        render = oracle.render_vector if vec else oracle.render
+        partial = torch.from_numpy(render(sh, raw=True))                 # this rank's raw S (double)
         calls = {"reduce": 0, "map": 0}
 
         def all_reduce(t):
@@ -66,18 +78,19 @@ def _worker(rank, world, port, q):
             t.copy_(-torch.expm1(-t))
 
         img = multi.combine_partials(partial, all_reduce, output_map)
-        raw = multi.combine_partials(torch.from_numpy(oracle.render(sh, raw=True)), all_reduce, None)
+        raw = multi.combine_partials(torch.from_numpy(render(sh, raw=True)), all_reduce, None)
         q.put((rank, img.numpy().copy(), raw.numpy().copy(), dict(calls)))
     finally:
         dist.destroy_process_group()
 
 
-def test_two_rank_gloo_sharded_render_equals_single_render():
+@pytest.mark.parametrize("vec", [False, True])
+def test_two_rank_gloo_sharded_render_equals_single_render(vec):
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, vec)) for r in range(2)]
     for p in procs:
         p.start()
     got = [q.get(timeout=300) for _ in procs]
@@ -85,7 +98,11 @@ def test_two_rank_gloo_sharded_render_equals_single_render():
         p.join(60)
         assert p.exitcode == 0
     w = workloads.make("C1", 20_000, width=96, height=64)
-    ref, ref_raw = oracle.render(w), oracle.render(w, raw=True)
+    if vec:
+        w.vec = np.random.RandomState(5).uniform(0, 1, (w.n, 3)).astype(np.float32)
+        ref, ref_raw = oracle.render_vector(w), oracle.render_vector(w, raw=True)
+    else:
+        ref, ref_raw = oracle.render(w), oracle.render(w, raw=True)
     assert ref.max() > 0.3
     for rank, img, raw, calls in got:
         assert calls == {"reduce": 2, "map": 1}

@@ -586,3 +586,32 @@ def test_p18_roi_equals_crop_of_full_frame(mode):
         x0, y0, x1, y1 = roi
         got = oracle.render(w, roi=roi)
         np.testing.assert_array_equal(got, full[y0:y1, x0:x1])
+
+
+# ------------------------------------------------------------------------------------------------
+# P19 (reading R20): negative absorption / emission / optical-depth modulation are unphysical but
+# "used as given": the slab solution of Eq. (1), holds for either sign of u = A tau.
+# RK4 integration of Eq. (1) with a negative A channel, a negative E channel and one negative I.
+# ------------------------------------------------------------------------------------------------
+def test_p19_rk4_absorb_negative_coefficients():
+    c = cam(eye=(0, 0, -12.0), fov=6.0, w=8, h=8)
+    pts = _disjoint_points()
+    pts[2] = pts[2][:4] + (-1.5,) + pts[2][5:]                   # negative I
+    lut_e = np.array([[0.2, -0.5, 0.9], [1.0, 0.3, -0.1]], np.float32)
+    lut_a = np.array([[1.5, 0.1, -0.6], [-0.05, 0.9, 2.0]], np.float32)
+    w = mk(pts, c, lut_e=lut_e, lut_a=lut_a, brightness=(1.3,), abs_brightness=(0.8,), mode=ABSORB)
+    E = np.float64(np.float32(1.3)) * _lerp(lut_e, w.colval)
+    A = np.float64(np.float32(0.8)) * _lerp(lut_a, w.colval)
+    ref = _ode_image(w, c, E, A, n_steps=12000)
+    out = oracle.render(w)
+    assert out.max() > 0.2 and out.min() < -0.05
+    np.testing.assert_allclose(out, ref, rtol=2e-7, atol=1e-9)
+    # additive mode is linear in E and I: S(-I) = -S(I)
+    wa = mk(pts, c, lut_e=lut_e, brightness=(1.3,))
+    pts_pos = [p[:4] + (abs(p[4]),) + p[5:] for p in pts]
+    Sa = oracle.render(wa, raw=True)
+    only = oracle.render(mk([pts[2]], c, lut_e=lut_e, brightness=(1.3,)), raw=True)
+    only_pos = oracle.render(mk([pts_pos[2]], c, lut_e=lut_e, brightness=(1.3,)), raw=True)
+    np.testing.assert_allclose(only, -only_pos, rtol=1e-15)
+    np.testing.assert_allclose(Sa, oracle.render(mk(pts_pos, c, lut_e=lut_e, brightness=(1.3,)), raw=True) - 2.0 * only_pos,
+                               rtol=1e-12, atol=1e-15)
