@@ -134,6 +134,27 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
                    const splotch_colormap *colormap, const splotch_params *params, float *out_rgb,
                    void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream);
 
+/* Multi-camera batch over ONE resident particle set: the orbit use case, stage (c) "render data"
+ * feeding stage (d) frame after frame (section 3 pipeline; BASELINE config 5 renders
+ * "an orbit of 8 camera positions over the resident particle set").
+ *   cameras      HOST array of n_cameras cameras; all must have the same width and height
+ *   out_rgb      DEVICE buffer of n_cameras images, image k at out_rgb + k * height * width * 3
+ *   frame_status DEVICE array of n_cameras * 4 uint64 (may be NULL): per frame {status (as int64),
+ *                visible, pairs, 0}, copied from the workspace status head after each frame, so that
+ *                one synchronisation after the call tells which frames (if any) needed more than
+ *                max_pairs pairs (those images are zero-filled; the others are complete)
+ *   workspace    ONE workspace of splotch_workspace_bytes(n, &cameras[0], params, max_pairs) bytes,
+ *                reused by every frame; max_pairs = the capacity every frame gets (use the largest
+ *                splotch_count_pairs over the cameras)
+ * Every argument is validated for EVERY camera before anything is enqueued: an invalid camera k
+ * fails the whole call with no work done.  Frame k is exactly splotch_render(cameras[k]); the
+ * frames are enqueued back to back on `stream` with no host synchronisation in between (the
+ * per-frame status copy is device to device).  Enqueue only; does not synchronise. */
+int splotch_render_batch(const splotch_particles *particles, int64_t n, const splotch_camera *cameras,
+                         int32_t n_cameras, const splotch_colormap *colormap, const splotch_params *params,
+                         float *out_rgb, uint64_t *frame_status, void *workspace, uint64_t workspace_bytes,
+                         uint64_t max_pairs, void *stream);
+
 /* Reads the status head the last call left in `workspace`.  SYNCHRONISES `stream`.
  * status: SPLOTCH_OK or SPLOTCH_ERR_WORKSPACE; visible: particles that passed culling;
  * pairs: (particle, block) pairs the scene needs.  Any output pointer may be NULL. */

@@ -30,7 +30,7 @@ SPLOTCH_FORCE_TENSOR = 4
 
 # every symbol include/splotch.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
-    "splotch_workspace_bytes", "splotch_render", "splotch_workspace_status", "splotch_count_pairs",
+    "splotch_workspace_bytes", "splotch_render", "splotch_render_batch", "splotch_workspace_status", "splotch_count_pairs",
     "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_tonemap_rgb8", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
     "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_tensor_stats", "splotch_debug_scan",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
@@ -194,6 +194,18 @@ def splotch_render(particles: splotch_particles, n: int, camera: splotch_camera,
            _lib().splotch_render(C.byref(particles), C.c_int64(n), C.byref(camera), C.byref(colormap), C.byref(params),
                                  _vp(_ptr(out_rgb)), _vp(_ptr(workspace)), C.c_uint64(workspace_bytes),
                                  C.c_uint64(max_pairs), _vp(_stream(stream))))
+
+
+def splotch_render_batch(particles: splotch_particles, n: int, cameras: Sequence[splotch_camera], colormap: splotch_colormap,
+                         params: splotch_params, out_rgb, frame_status, workspace, workspace_bytes: int, max_pairs: int,
+                         stream=None) -> None:
+    """K cameras over one resident particle set: out_rgb holds K images back to back, frame_status (device, K*4 uint64
+    as int64 tensor, or None) receives per frame (status, visible, pairs, 0).  Enqueue only."""
+    arr = (splotch_camera * max(len(cameras), 1))(*cameras)
+    _check("splotch_render_batch",
+           _lib().splotch_render_batch(C.byref(particles), C.c_int64(n), arr, C.c_int32(len(cameras)), C.byref(colormap),
+                                       C.byref(params), _vp(_ptr(out_rgb)), _vp(_ptr(frame_status)), _vp(_ptr(workspace)),
+                                       C.c_uint64(workspace_bytes), C.c_uint64(max_pairs), _vp(_stream(stream))))
 
 
 def splotch_workspace_status(workspace, stream=None):

@@ -409,6 +409,44 @@ int splotch_render(const splotch_particles *particles, int64_t n, const splotch_
     return SPLOTCH_OK;
 }
 
+namespace splotch { namespace {
+__global__ void copy_frame_status_kernel(const WorkHead *head, uint64_t *dst)
+{
+    dst[0] = (uint64_t)(int64_t)head->status;
+    dst[1] = head->visible;
+    dst[2] = head->pairs;
+    dst[3] = 0ull;
+}
+} }
+
+int splotch_render_batch(const splotch_particles *particles, int64_t n, const splotch_camera *cameras, int32_t n_cameras,
+                         const splotch_colormap *colormap, const splotch_params *params, float *out_rgb,
+                         uint64_t *frame_status, void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream)
+{
+    if (!cameras || n_cameras < 0 || (n_cameras > 0 && !out_rgb)) return SPLOTCH_ERR_INVALID_ARG;
+    if (frame_status && (reinterpret_cast<uintptr_t>(frame_status) & 7u)) return SPLOTCH_ERR_INVALID_ARG;
+    // validate everything for every camera before enqueueing anything
+    for (int32_t k = 0; k < n_cameras; ++k) {
+        if (cameras[k].width != cameras[0].width || cameras[k].height != cameras[0].height) return SPLOTCH_ERR_INVALID_ARG;
+        Ctx c;
+        const int rc = setup(particles, n, &cameras[k], colormap, params, kBlockShift, workspace, workspace_bytes, max_pairs,
+                             true, stream, &c);
+        if (rc) return rc;
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    for (int32_t k = 0; k < n_cameras; ++k) {
+        const size_t frame = (size_t)cameras[k].width * cameras[k].height * 3;
+        const int rc = splotch_render(particles, n, &cameras[k], colormap, params, out_rgb + (size_t)k * frame, workspace,
+                                      workspace_bytes, max_pairs, stream);
+        if (rc) return rc;
+        if (frame_status) {
+            copy_frame_status_kernel<<<1, 1, 0, st>>>(reinterpret_cast<const WorkHead *>(workspace), frame_status + 4 * (size_t)k);
+            SPLOTCH_LAUNCH_CHECK();
+        }
+    }
+    return SPLOTCH_OK;
+}
+
 int splotch_profile_enable(int on)
 {
     std::lock_guard<std::mutex> lock(g_prof_mutex);

@@ -117,6 +117,31 @@ class Scene:
                 raise B.SplotchError(f"splotch_render (scene needs {pairs} pairs, max_pairs={self.max_pairs})", status)
         return out
 
+    def render_batch(self, cams=None, mode: Optional[int] = None, raw: bool = False, out: Optional[torch.Tensor] = None,
+                     check: bool = True):
+        """One splotch_render_batch over `cams` (default: every camera of the workload: the orbit).  Returns
+        (images (K, H, W, 3) float32 CUDA tensor, frame_status (K, 4) int64 CUDA tensor: status, visible, pairs, 0).
+        The workspace is sized once for the largest pair count over the cameras."""
+        cams = list(self.w.cameras if cams is None else cams)
+        K = len(cams)
+        cs = [_camera_struct(c) for c in cams]
+        ps = self.params(mode, raw)
+        if self.workspace is None or self.max_pairs == 0:
+            worst = max(self.count_pairs(c, mode)[0] for c in cams) if K else 0
+            self.reserve(cams[0] if K else None, mode, max_pairs=worst + 1024)
+        H, W = (cams[0].height, cams[0].width) if K else (0, 0)
+        if out is None:
+            out = torch.empty((K, H, W, 3), dtype=torch.float32, device=self.device)
+        status = torch.zeros((max(K, 1), 4), dtype=torch.int64, device=self.device)
+        B.splotch_render_batch(self.particles(), self.n, cs, self.colormap(), ps, out, status, self._aligned(self.workspace),
+                               self.workspace.numel() - 256, self.max_pairs)
+        if check:
+            bad = [(k, int(r[2])) for k, r in enumerate(status[:K].cpu().tolist()) if r[0] != B.SPLOTCH_OK]
+            if bad:
+                raise B.SplotchError(f"splotch_render_batch (frames {bad} need more than max_pairs={self.max_pairs})",
+                                     B.SPLOTCH_ERR_WORKSPACE)
+        return out, status[:K]
+
     def stats(self, cam=None, mode: Optional[int] = None, bin_shift: int = 6):
         """(visible, pairs at bin_shift, pixel updates U); synchronises."""
         cam = cam or self.w.camera

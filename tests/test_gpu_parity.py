@@ -403,6 +403,47 @@ def test_repeat_calls_and_orbit_cameras(B):
     np.testing.assert_allclose(again, first, rtol=2e-5, atol=1e-6)   # atomics and MMA batching: order of partial sums may differ
 
 
+def test_render_batch_orbit_matches_oracle_per_camera(B):
+    """splotch_render_batch (f4, PAPER.md:81): the 8-camera orbit of C5 in ONE call over the resident particle set;
+    every frame against the oracle, and bit-for-bit equal to what it is defined as (splotch_render per camera, ALU path:
+    deterministic up to the order of atomics, so compared within rounding); per-frame status words."""
+    w = workloads.make("C5", 200_000, width=192, height=160)
+    sc = _scene(w, tensor=False)
+    imgs, status = sc.render_batch(raw=True)
+    torch.cuda.synchronize()
+    st = status.cpu().numpy()
+    assert imgs.shape == (8, 160, 192, 3) and (st[:, 0] == 0).all() and (st[:, 3] == 0).all()
+    for j, cm in enumerate(w.cameras):
+        ref = oracle.render(w, camera=cm, raw=True)
+        _tol_check(imgs[j].cpu().numpy(), ref, f"C5 batch camera {j}")
+        pairs, vis = sc.count_pairs(cm)
+        assert int(st[j, 1]) == vis and int(st[j, 2]) == pairs
+    single = sc.render(cam=w.cameras[5], raw=True).cpu().numpy()
+    np.testing.assert_allclose(imgs[5].cpu().numpy(), single, rtol=2e-5, atol=1e-6)
+    # a capacity that only some frames exceed: those frames are zero with an error status, the others complete
+    pairs_all = [sc.count_pairs(cm)[0] for cm in w.cameras]
+    cap = sorted(pairs_all)[3]
+    sc.max_pairs = cap
+    imgs2, status2 = sc.render_batch(raw=True, check=False)
+    st2 = status2.cpu().numpy()
+    for j, p in enumerate(pairs_all):
+        if p > cap:
+            assert st2[j, 0] == B.SPLOTCH_ERR_WORKSPACE and float(imgs2[j].abs().max()) == 0.0
+        else:
+            assert st2[j, 0] == 0
+            np.testing.assert_allclose(imgs2[j].cpu().numpy(), imgs[j].cpu().numpy(), rtol=2e-5, atol=1e-6)
+    with pytest.raises(B.SplotchError):
+        sc.render_batch(raw=True)
+    # mixed image sizes are rejected before anything is enqueued; an empty batch is a no-op
+    from paper_1004_1302_b200.scene import _camera_struct
+    cs = [_camera_struct(w.cameras[0]), B.make_camera((0, 0, -3), (0, 0, 0), (0, 1, 0), 30.0, 100, 100)]
+    with pytest.raises(B.SplotchError):
+        B.splotch_render_batch(sc.particles(), sc.n, cs, sc.colormap(), sc.params(), imgs, None, sc._aligned(sc.workspace),
+                               sc.workspace.numel() - 256, sc.max_pairs)
+    B.splotch_render_batch(sc.particles(), sc.n, [], sc.colormap(), sc.params(), imgs, None, sc._aligned(sc.workspace),
+                           sc.workspace.numel() - 256, sc.max_pairs)
+
+
 def test_stats_counts(B):
     w = workloads.make("C1")
     sc = _scene(w)
