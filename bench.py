@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- the Splotch render hot path on B200: Mparticles/s and roofline fractions.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--r-median X] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (transform/cull/colour -> bin -> rasterise -> output
 map) over the resident synthetic particle set of the workload.  The default workload is C3, the
-100M-particle additive config BASELINE.json's north_star quotes its target on.  One JSON line is
-printed on stdout (rank 0); everything else goes to stderr.
+100M-particle additive config BASELINE.json's north_star quotes its target on.  For C5 a step is the
+whole 8-camera orbit (one splotch_render_batch).  --r-median X renders C3's geometry with another median
+smoothing length (the footprint sweep of SURVEY.md 8(d): where the path becomes HBM-bound).  One JSON
+line is printed on stdout (rank 0); everything else goes to stderr.
 
 N > 1 (torchrun, one rank per GPU): additive mode shards by particles exactly like the paper's
 MPI layer: every rank renders its own particle set into a raw-S partial image,
@@ -106,9 +108,13 @@ class ClockSampler:
                     reasons=sorted(reasons), samples=len(sm))
 
 
-def make_workload(name: str, n, rank: int):
+def make_workload(name: str, n, rank: int, r_median=None):
     import workloads
     kw = {}
+    if r_median is not None:
+        if name != "C3":
+            raise SystemExit("--r-median applies to C3's geometry only")
+        kw["r_median"] = float(r_median)
     if rank > 0:
         kw["seed"] = {"C1": 1004130201, "C2": 1004130202, "C3": 1004130203, "C4": 1004130202, "C5": 1004130205}[name] + 1000 * rank
     t = time.time()
@@ -135,7 +141,7 @@ def oracle_sample(w, target_seconds: float):
 def run_reference(args):
     """--impl reference: the CPU oracle (as it stands) on a bounded sample of the same workload."""
     import oracle
-    w = make_workload(args.workload, args.n, 0)
+    w = make_workload(args.workload, args.n, 0, args.r_median)
     budget = 150.0 / max(1, args.steps + args.warmup)
     ws, stride, cores = oracle_sample(w, min(25.0, budget))
     for _ in range(args.warmup):
@@ -169,6 +175,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--force-tensor", action="store_true", help="additive mode: SPLOTCH_FORCE_TENSOR")
     ap.add_argument("--no-tensor", action="store_true", help="additive mode: SPLOTCH_NO_TENSOR (everything on the FP32 ALUs)")
+    ap.add_argument("--r-median", type=float, default=None,
+                    help="C3 only: median smoothing length (default 0.005 = the config); the footprint sweep uses 0.0015 / 0.0005 / 0.00015")
+    ap.add_argument("--single-frame", action="store_true", help="C5: time camera 0 only instead of the 8-camera orbit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -193,25 +202,39 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     peaks = read_peaks()
-    w = make_workload(args.workload, args.n, rank)
+    w = make_workload(args.workload, args.n, rank, args.r_median)
     if world > 1 and w.mode != 0:
         raise SystemExit("multi-GPU sharding is defined for the additive mode only (DESIGN.md 'Multi-GPU')")
-    cam = w.camera
-    sc = Scene(w, dev)
+    cams = list(w.cameras) if (len(w.cameras) > 1 and not args.single_frame) else [w.camera]
+    n_frames = len(cams)                                   # C5: the 8-camera orbit is ONE step
+    cam = cams[0]
+    if world > 1:
+        from paper_1004_1302_b200.multi import ShardedScene
+        sharded = ShardedScene(w, dev)                     # every rank: its own particle set (weak scaling) + one all-reduce
+        sc = sharded.scene
+    else:
+        sc = Scene(w, dev)
     sc.tensor = False if args.no_tensor else True if args.force_tensor else None
-    vis, pairs, updates = sc.stats()
-    upd_tensor, tensor_on, tensor_share = sc.tensor_stats() if w.mode == 0 else (0, 0, 0.0)
-    sc.reserve(max_pairs=pairs + 1024)
-    log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g}, "
+    per_cam = [sc.stats(c) for c in cams]                  # (visible, pairs, updates) per camera
+    vis, pairs = per_cam[0][0], max(p for _, p, _ in per_cam)
+    updates = float(np.mean([u for _, _, u in per_cam]))   # per frame
+    if w.mode == 0:
+        ts = [sc.tensor_stats(c) for c in cams]
+        upd_tensor, tensor_on, tensor_share = float(np.mean([t[0] for t in ts])), ts[0][1], float(np.mean([t[2] for t in ts]))
+    else:
+        upd_tensor, tensor_on, tensor_share = 0, 0, 0.0
+    sc.reserve(cam, max_pairs=pairs + 1024)
+    log(f"[bench] rank {rank}: visible {vis}, pairs {pairs}, pixel updates U {updates:.4g} per frame, frames per step {n_frames}, "
         f"workspace {sc.workspace.numel() / 2**30:.2f} GiB")
-    out = torch.empty((cam.height, cam.width, 3), dtype=torch.float32, device=dev)
-    raw = world > 1
+    out = torch.empty((n_frames, cam.height, cam.width, 3), dtype=torch.float32, device=dev)
 
     def step():
-        sc.render(cam, raw=raw, out=out, check=False)
-        if world > 1:                              # one collective reduction of the partial images
-            dist.all_reduce(out)
-            B.splotch_normalize(out, out, out.numel())
+        if world > 1:                              # one collective reduction of the partial images, then the output map
+            sharded.render(cam, out=out[0], check=False)
+        elif n_frames > 1:
+            sc.render_batch(cams, out=out, check=False)
+        else:
+            sc.render(cam, out=out[0], check=False)
 
     def barrier():
         if world > 1:
@@ -229,14 +252,15 @@ def main():
     time.sleep(0.25)
     launches0 = B.splotch_launch_count()
     B.splotch_profile_enable(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    e0.record()
-    for _ in range(args.steps):
+    ev[0].record()
+    for k in range(args.steps):
         step()
-    e1.record()
+        ev[k + 1].record()                         # one event per step: median and best beside the mean
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = ev[0].elapsed_time(ev[-1])
+    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     stage_ms, prof_calls = B.splotch_profile_read()
     B.splotch_profile_enable(False)
     launches = B.splotch_launch_count() - launches0
@@ -249,8 +273,9 @@ def main():
         tl = torch.tensor([launches], dtype=torch.int64, device=dev)
         dist.all_reduce(tl)
         launches = int(tl.item())
-    total_particles = w.n * world
+    total_particles = w.n * world * n_frames       # every frame renders all N input particles
     value = total_particles / (ms_step * 1e-3) / 1e6
+    ms_frame = ms_step / n_frames
 
     # ---- rooflines of the rasteriser (K3): plain FP32 ALU kernel, and in the additive mode the tensor-core kernel ----
     tensor_ms, alu_ms = stage_ms[3], stage_ms[4]
@@ -264,7 +289,7 @@ def main():
     alu_achieved = upd_alu * c_ops / (alu_ms * 1e-3) / 1e12 if alu_ms > 0 else 0.0
     alu_roof = dict(bound="alu", kernel=alu_kernel, achieved=alu_achieved, peak=alu_peak, unit="Tlane-op/s",
                     frac=alu_achieved / alu_peak if alu_peak else None, traffic=read_traffic(w.name, alu_kernel),
-                    kernel_ms=alu_ms, kernel_share_of_step=alu_ms / ms_step if ms_step else None,
+                    kernel_ms=alu_ms, kernel_share_of_step=alu_ms / ms_frame if ms_frame else None,
                     updates_per_launch=upd_alu, algorithmic_lane_ops_per_update=c_ops,
                     peak_source=f"{sm_count} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} clock)")
     tensor_roof = None
@@ -273,7 +298,7 @@ def main():
         t_achieved = 2.0 * 3.0 * upd_tensor / (tensor_ms * 1e-3) / 1e12            # one multiply-add per channel per update
         tensor_roof = dict(bound="tensor", kernel="raster_additive_mma_kernel", achieved=t_achieved, peak=tf32_peak,
                            unit="TFLOP/s", frac=t_achieved / tf32_peak, traffic=read_traffic(w.name, "raster_additive_mma_kernel"),
-                           kernel_ms=tensor_ms, kernel_share_of_step=tensor_ms / ms_step, updates_per_launch=upd_tensor,
+                           kernel_ms=tensor_ms, kernel_share_of_step=tensor_ms / ms_frame, updates_per_launch=upd_tensor,
                            algorithmic_flops_per_update=6.0,
                            executed_over_algorithmic=4.0,   # 3 split-TF32 products x 128/96 padded accumulator rows
                            peak_source=f"0.5 x sustained dense BF16 cuBLAS throughput ({peaks['source']}) = TF32 dense")
@@ -285,58 +310,103 @@ def main():
                         tensor_share_estimate=tensor_share, tensor_cores_used=bool(tensor_used),
                         note="all K3 updates x algorithmic lane-ops / (tensor + ALU kernel time): what an ALU-only "
                              "rasteriser would have to sustain to match")
-    algo_bytes = w.n * w.bytes_per_particle + cam.width * cam.height * 12
-    hbm_gbs = algo_bytes / (ms_step * 1e-3) / 1e9
+    algo_bytes = w.n * w.bytes_per_particle + cam.width * cam.height * 12       # per frame
+    hbm_gbs = algo_bytes / (ms_frame * 1e-3) / 1e9
     hbm = dict(algorithmic_bytes_per_step=algo_bytes, achieved_gbs=hbm_gbs, frac_of_measured=hbm_gbs / peaks["hbm_gbs"],
                frac_of_nominal_8TBs=hbm_gbs / 8000.0, peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"])
 
-    # ---- end to end through the C ABI with host buffers (H2D + render + D2H inside the call) ----
+    # front end (K1 and the lists) against the HBM roofline by the bytes these kernels themselves must move
+    rec_bytes = 48 if w.mode else 32
+    k1_bytes = w.n * (w.bytes_per_particle + rec_bytes + 4 + (4 if w.mode else 0))    # inputs read; record, packed bin box (, depth key) written
+    list_bytes = w.n * 4 + per_cam[0][1] * 4                                          # packed bin boxes read, pair list written (additive)
+    frontend = dict(project_ms=stage_ms[0], project_bytes=k1_bytes,
+                    project_frac_of_hbm=k1_bytes / (stage_ms[0] * 1e-3) / 1e9 / peaks["hbm_gbs"] if stage_ms[0] > 0 else None,
+                    lists_ms=stage_ms[2], lists_bytes=list_bytes if w.mode == 0 else None,
+                    lists_frac_of_hbm=(list_bytes / (stage_ms[2] * 1e-3) / 1e9 / peaks["hbm_gbs"]) if (w.mode == 0 and stage_ms[2] > 0) else None,
+                    frontend_share_of_frame=(stage_ms[0] + stage_ms[1] + stage_ms[2]) / ms_frame if ms_frame else None)
+
+    # ---- end to end through the C ABI with host buffers: every frame copies its inputs H2D and its image D2H ----
     e2e = None
     if not args.no_e2e and world == 1:
         hb = sc.host_buffers()
         out_host = torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory()
         sc.workspace = None
         torch.cuda.empty_cache()
-        _, hws = sc.render_host(hb, cam, out_host=out_host, max_pairs=pairs + 1024)
-        n_e2e = max(1, min(args.steps, 3))
+        mp = pairs + 1024
+        # (a) one call at a time: splotch_render_host (copies, render, copy back, synchronise)
+        _, hws = sc.render_host(hb, cam, out_host=out_host, max_pairs=mp)
+        n_serial = max(1, min(args.steps, 3))
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            sc.render_host(hb, cam, out_host=out_host, max_pairs=pairs + 1024, workspace=hws)
-        dt = (time.perf_counter() - t0) / n_e2e
-        e2e = dict(value=w.n / dt / 1e6, unit="Mparticles/s", h2d_bytes_per_step=sc.h2d_bytes(),
-                   d2h_bytes_per_step=cam.width * cam.height * 12, ms_per_step=dt * 1e3, steps=n_e2e,
-                   call="splotch_render_host (pinned host buffers; copies inside the timed call)")
+        for _ in range(n_serial):
+            sc.render_host(hb, cam, out_host=out_host, max_pairs=mp, workspace=hws)
+        dt_serial = (time.perf_counter() - t0) / n_serial
         del hws
+        torch.cuda.empty_cache()
+        # (b) a stream of frames, two in flight (splotch_render_host_async on two streams / workspaces): the copies of
+        #     frame k + 1 run on the copy engines while frame k is rasterised; every frame still moves all its bytes
+        free, _ = torch.cuda.mem_get_info()
+        need = 2 * B.splotch_workspace_bytes_host(w.n, B.make_camera(cam.eye, cam.lookat, cam.up, cam.fov_deg, cam.width, cam.height),
+                                                  B.make_colormap(hb["lut_e"], hb["lut_a"], sc.n_entries, sc.n_types), sc.params(), mp)
+        dt_pipe, n_pipe = None, 0
+        if free > need + (2 << 30):
+            sc.render_host_pipelined(hb, 2, cam, max_pairs=mp)                       # warm-up: allocates the two slots
+            n_pipe = max(4, min(2 * args.steps, 10))
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            sc.render_host_pipelined(hb, n_pipe, cam, max_pairs=mp)
+            dt_pipe = (time.perf_counter() - t0) / n_pipe
+            sc._pipe = None
+            torch.cuda.empty_cache()
+        dt = dt_pipe if dt_pipe is not None else dt_serial
+        e2e = dict(value=w.n / dt / 1e6, unit="Mparticles/s", h2d_bytes_per_step=sc.h2d_bytes(),
+                   d2h_bytes_per_step=cam.width * cam.height * 12, ms_per_step=dt * 1e3, steps=n_pipe if dt_pipe is not None else n_serial,
+                   call=("splotch_render_host_async, two frames in flight on two streams (pinned host buffers; every frame "
+                         "copies its inputs H2D and its image D2H inside the timed region)") if dt_pipe is not None else
+                        "splotch_render_host (pinned host buffers; copies inside the timed call)",
+                   serial=dict(value=w.n / dt_serial / 1e6, ms_per_step=dt_serial * 1e3, steps=n_serial,
+                               call="splotch_render_host, one synchronous call at a time (latency of one frame)"),
+                   frames_per_step=1, note="per frame (camera 0)" if n_frames > 1 else None)
     elif world > 1:
         e2e = dict(value=None, unit="Mparticles/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0,
                    note="end-to-end host-buffer path is measured at N=1")
 
-    # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only ----
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only; best and median of 3 ----
     cpu = None
     if not args.no_cpu_baseline and world == 1 and rank == 0:
         import oracle
-        ws_, stride, cores = oracle_sample(w, 15.0)
-        t0 = time.time()
-        oracle.render(ws_)
-        dt = time.time() - t0
-        cpu = dict(value=ws_.n / dt / 1e6, unit="Mparticles/s", cores=cores, kind="oracle", seconds=dt,
+        ws_, stride, cores = oracle_sample(w, 7.0)
+        times = []
+        for _ in range(3):
+            t0 = time.time()
+            oracle.render(ws_)
+            times.append(time.time() - t0)
+        best, med = min(times), float(np.median(times))
+        cpu = dict(value=ws_.n / best / 1e6, unit="Mparticles/s", cores=cores, kind="oracle", seconds=best,
+                   median_value=ws_.n / med / 1e6, runs=3,
                    sample=f"1-in-{stride} particle-strided subsample ({ws_.n} particles) of {w.name} at full resolution "
-                          f"(subsample measurement)")
+                          f"(subsample measurement; best of 3, median beside it)")
 
     if rank == 0:
+        wl = f"{w.name}: {w.n} particles/GPU, {cam.width}x{cam.height}, {'absorb' if w.mode else 'additive'} mode, f={w.support_f}"
+        if args.r_median is not None:
+            wl += f", median r {args.r_median} (footprint sweep; the config has 0.005)"
+        if n_frames > 1:
+            wl += f", orbit of {n_frames} cameras per step (splotch_render_batch)"
         line = dict(metric=METRIC, value=value, unit="Mparticles/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
-                    ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                    ms_per_step=ms_step, ms_per_step_median=float(np.median(per_step)), ms_per_step_best=float(min(per_step)),
+                    higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                     data="synthetic",
-                    config=dict(workload=f"{w.name}: {w.n} particles/GPU, {cam.width}x{cam.height}, "
-                                         f"{'absorb' if w.mode else 'additive'} mode, f={w.support_f}",
+                    config=dict(workload=wl,
                                 parallelism=f"particle shards x{world} + all-reduce of raw S" if world > 1 else "single GPU",
                                 l2="inputs (particle arrays + splat records + pair list) exceed the 126 MB L2 many times over; no flush needed",
-                                seed=w.seed, visible=vis, pairs=pairs, pixel_updates=updates,
-                                pixels_per_s=cam.width * cam.height / (ms_step * 1e-3),
-                                updates_per_s=updates * world / (ms_step * 1e-3)),
+                                seed=w.seed, visible=vis, pairs=pairs, pixel_updates=updates, updates_per_particle=updates / w.n,
+                                frames_per_step=n_frames, ms_per_frame=ms_frame,
+                                pixels_per_s=cam.width * cam.height / (ms_frame * 1e-3),
+                                updates_per_s=updates * world / (ms_frame * 1e-3)),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline,
                     roofline_alu=alu_roof, roofline_tensor=tensor_roof, raster_alu_equivalent=raster_equiv, hbm_roofline=hbm,
+                    frontend=frontend,
                     stage_ms=dict(zip(["project_count", "offsets", "lists", "raster_tensor", "raster_alu", "output_map"], stage_ms)),
                     cpu_baseline=cpu)
         print(json.dumps(line), flush=True)

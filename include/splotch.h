@@ -204,6 +204,19 @@ int splotch_render_host(const splotch_particles *particles_host, int64_t n, cons
                         float *out_rgb_host, void *workspace, uint64_t workspace_bytes, uint64_t max_pairs,
                         void *stream);
 
+/* The same, ENQUEUE ONLY: host-to-device copies, render and the device-to-host copy of the image are
+ * enqueued on `stream` and the call returns.  The host buffers must stay valid and unchanged (and
+ * out_rgb_host unread) until the stream has passed the call; splotch_workspace_status(workspace,
+ * stream, ...) then synchronises and returns the status head (it sits at the start of the workspace
+ * in this layout too).  With two streams and two workspaces a sequence of frames (the snapshots of a
+ * time-dependent run: stage (a) "read" feeding (c) "render") is pipelined: the copies of
+ * frame k + 1 run on the copy engines while frame k is rasterised.  Pinned host memory is required
+ * for the copies to be asynchronous. */
+int splotch_render_host_async(const splotch_particles *particles_host, int64_t n, const splotch_camera *camera,
+                              const splotch_colormap *colormap_host, const splotch_params *params,
+                              float *out_rgb_host, void *workspace, uint64_t workspace_bytes, uint64_t max_pairs,
+                              void *stream);
+
 /* ------------------------------------------------------------------------------------------
  * Test-only exports for the bit-exact checks (north_star: "Tile/bin indices and counts must be
  * bit-exact").  They run the SAME kernels as splotch_render with extra outputs.

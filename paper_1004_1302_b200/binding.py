@@ -31,7 +31,7 @@ SPLOTCH_FORCE_TENSOR = 4
 # every symbol include/splotch.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
     "splotch_workspace_bytes", "splotch_render", "splotch_render_batch", "splotch_workspace_status", "splotch_count_pairs",
-    "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_tonemap_rgb8", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_debug_project",
+    "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_tonemap_rgb8", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_render_host_async", "splotch_debug_project",
     "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_tensor_stats", "splotch_debug_scan",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
     "splotch_last_cuda_error", "splotch_version", "splotch_profile_enable", "splotch_profile_read",
@@ -256,6 +256,16 @@ def splotch_render_host(particles_host: splotch_particles, n: int, camera: splot
            _lib().splotch_render_host(C.byref(particles_host), C.c_int64(n), C.byref(camera), C.byref(colormap_host),
                                       C.byref(params), _vp(_ptr(out_rgb_host)), _vp(_ptr(workspace)),
                                       C.c_uint64(workspace_bytes), C.c_uint64(max_pairs), _vp(_stream(stream))))
+
+
+def splotch_render_host_async(particles_host: splotch_particles, n: int, camera: splotch_camera,
+                              colormap_host: splotch_colormap, params: splotch_params, out_rgb_host, workspace,
+                              workspace_bytes: int, max_pairs: int, stream=None) -> None:
+    """Enqueue only: H2D copies, render, D2H copy of the image on `stream`; check later with splotch_workspace_status."""
+    _check("splotch_render_host_async",
+           _lib().splotch_render_host_async(C.byref(particles_host), C.c_int64(n), C.byref(camera), C.byref(colormap_host),
+                                            C.byref(params), _vp(_ptr(out_rgb_host)), _vp(_ptr(workspace)),
+                                            C.c_uint64(workspace_bytes), C.c_uint64(max_pairs), _vp(_stream(stream))))
 
 
 def splotch_debug_project(particles, n, camera, colormap, params, workspace, workspace_bytes, sx, sy, sigma_s, R, zkey,

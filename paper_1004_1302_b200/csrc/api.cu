@@ -153,15 +153,16 @@ int bits_for(int n_bins)
 // workspace layout
 // ---------------------------------------------------------------------------------------------
 struct Layout {
-    uint64_t head, records, bin_count, bin_cursor, bin_offset, unit_prefix, scan_scratch, list;
+    uint64_t head, records, bin_count, bin_cursor, bin_offset, unit_prefix, scan_scratch, list, bin_diff, bin_diff_bytes, binsw;
     // absorb mode
     uint64_t zkeys, ids, zkeys_tmp, ids_tmp, sort_scratch, pair_count, pair_offset, pair_bin, pair_id, pair_bin_tmp,
         partials;
     uint64_t total;
 };
 
-Layout make_layout(int64_t n, int n_bins, int mode, uint64_t max_pairs, bool want_partials)
+Layout make_layout(int64_t n, int nbx, int nby, int mode, uint64_t max_pairs, bool want_partials)
 {
+    const int n_bins = nbx * nby;
     Layout L;
     memset(&L, 0, sizeof(L));
     uint64_t off = 0;
@@ -173,6 +174,9 @@ Layout make_layout(int64_t n, int n_bins, int mode, uint64_t max_pairs, bool wan
     const uint64_t nn = (uint64_t)(n > 0 ? n : 1);
     L.head = take(256);
     L.records = take(nn * (mode == SPLOTCH_ABSORB ? sizeof(SplatAbs) : sizeof(SplatAdd)));
+    L.bin_diff_bytes = (uint64_t)(nbx + 1) * (uint64_t)(nby + 1) * 4;
+    L.bin_diff = take(L.bin_diff_bytes);
+    L.binsw = take(nn * 4);
     L.bin_count = take((uint64_t)n_bins * 4);
     L.bin_cursor = take((uint64_t)n_bins * 4);
     L.bin_offset = take((uint64_t)(n_bins + 1) * 8);
@@ -227,7 +231,7 @@ int setup(const splotch_particles *particles, int64_t n, const splotch_camera *c
     if (max_pairs >= (1ull << 32)) return SPLOTCH_ERR_LIMIT;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return SPLOTCH_ERR_INVALID_ARG;
     c->n_bins = c->rc.nbx * c->rc.nby;
-    c->L = make_layout(n, c->n_bins, params->mode, max_pairs, want_partials);
+    c->L = make_layout(n, c->rc.nbx, c->rc.nby, params->mode, max_pairs, want_partials);
     if (workspace_bytes < c->L.total) return SPLOTCH_ERR_WORKSPACE;
     c->ws = reinterpret_cast<char *>(workspace);
     c->st = reinterpret_cast<cudaStream_t>(stream);
@@ -239,14 +243,17 @@ int run_front(const Ctx &c, const splotch_particles *particles, int64_t n, const
               uint64_t max_pairs, uint32_t chunk, const DebugProjectOut *dbg, bool profiled = false)
 {
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.head, 0, 256, c.st));
+    SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_diff, 0, (size_t)c.L.bin_diff_bytes, c.st));
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_count, 0, (size_t)c.n_bins * 4, c.st));
     SPLOTCH_CUDA_TRY(cudaMemsetAsync(c.ws + c.L.bin_cursor, 0, (size_t)c.n_bins * 4, c.st));
     ParticlePtrs pp = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
     if (n > 0) pp = { particles->x, particles->y, particles->z, particles->r, particles->I, particles->colval, particles->type,
                       particles->vr, particles->vg, particles->vb };
     int rc = launch_project(pp, n, c.cam, c.rc, cm->emission, cm->absorption, c.ws + c.L.records,
-                            c.at<uint32_t>(c.L.bin_count), c.rc.mode == SPLOTCH_ABSORB ? c.at<uint32_t>(c.L.zkeys) : nullptr,
-                            c.head(), dbg, c.st);
+                            c.at<int>(c.L.bin_diff), c.at<uint32_t>(c.L.binsw),
+                            c.rc.mode == SPLOTCH_ABSORB ? c.at<uint32_t>(c.L.zkeys) : nullptr, c.head(), dbg, c.st);
+    if (rc) return rc;
+    rc = launch_bins_from_diff(c.at<int>(c.L.bin_diff), c.rc, c.at<uint32_t>(c.L.bin_count), c.st);
     if (rc) return rc;
     if (profiled) prof_mark(1, c.st);
     rc = launch_scan_u32_u64(c.at<uint32_t>(c.L.bin_count), c.at<uint64_t>(c.L.bin_offset), c.n_bins,
@@ -264,7 +271,7 @@ int run_lists(const Ctx &c, int64_t n, uint64_t max_pairs, uint32_t **list_out)
     *list_out = c.at<uint32_t>(c.L.list);
     if (n <= 0 || max_pairs == 0) return SPLOTCH_OK;
     if (c.rc.mode == SPLOTCH_ADDITIVE)
-        return launch_scatter(c.ws + c.L.records, rec_bytes, n, c.rc, c.at<uint64_t>(c.L.bin_offset),
+        return launch_scatter(c.at<uint32_t>(c.L.binsw), n, c.rc, c.at<uint64_t>(c.L.bin_offset),
                               c.at<uint32_t>(c.L.bin_cursor), c.at<uint32_t>(c.L.list), max_pairs, c.head(), c.st);
     // a7: order the particles by (depth key, index): stable LSD sort of the keys with iota values
     int rc = launch_iota(c.at<uint32_t>(c.L.ids), n, c.st);
@@ -340,7 +347,7 @@ int splotch_workspace_bytes(int64_t n, const splotch_camera *camera, const splot
     rc = make_render_const(camera, nullptr, params, kBlockShift, &r);
     if (rc) return rc;
     if (max_pairs >= (1ull << 32)) return SPLOTCH_ERR_LIMIT;
-    *bytes = make_layout(n, r.nbx * r.nby, params->mode, max_pairs, true).total;
+    *bytes = make_layout(n, r.nbx, r.nby, params->mode, max_pairs, true).total;
     return SPLOTCH_OK;
 }
 
@@ -355,7 +362,7 @@ int splotch_debug_workspace_bytes(int64_t n, const splotch_camera *camera, const
     rc = make_render_const(camera, nullptr, params, bin_shift, &r);
     if (rc) return rc;
     if (max_members >= (1ull << 32)) return SPLOTCH_ERR_LIMIT;
-    *bytes = make_layout(n, r.nbx * r.nby, params->mode, max_members, false).total;
+    *bytes = make_layout(n, r.nbx, r.nby, params->mode, max_members, false).total;
     return SPLOTCH_OK;
 }
 
@@ -562,9 +569,9 @@ int splotch_workspace_bytes_host(int64_t n, const splotch_camera *camera, const 
     return SPLOTCH_OK;
 }
 
-int splotch_render_host(const splotch_particles *ph, int64_t n, const splotch_camera *camera,
-                        const splotch_colormap *cmh, const splotch_params *params, float *out_rgb_host,
-                        void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream)
+int splotch_render_host_async(const splotch_particles *ph, int64_t n, const splotch_camera *camera,
+                              const splotch_colormap *cmh, const splotch_params *params, float *out_rgb_host,
+                              void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream)
 {
     if (!out_rgb_host || !workspace || !params) return SPLOTCH_ERR_INVALID_ARG;
     if (ph && (ph->vr || !ph->colval) && n > 0) return SPLOTCH_ERR_INVALID_ARG;     // host path: scalar colouring only
@@ -599,10 +606,18 @@ int splotch_render_host(const splotch_particles *ph, int64_t n, const splotch_ca
     rc = splotch_render(&pd, n, camera, &cmd, params, img, ws + H.inner, inner, max_pairs, stream);
     if (rc) return rc;
     SPLOTCH_CUDA_TRY(cudaMemcpyAsync(out_rgb_host, img, (size_t)camera->width * camera->height * 12, cudaMemcpyDeviceToHost, st));
-    SPLOTCH_CUDA_TRY(cudaStreamSynchronize(st));
-    WorkHead h;
-    SPLOTCH_CUDA_TRY(cudaMemcpy(&h, ws + H.inner, sizeof(h), cudaMemcpyDeviceToHost));
-    return h.status;
+    return SPLOTCH_OK;
+}
+
+int splotch_render_host(const splotch_particles *ph, int64_t n, const splotch_camera *camera,
+                        const splotch_colormap *cmh, const splotch_params *params, float *out_rgb_host,
+                        void *workspace, uint64_t workspace_bytes, uint64_t max_pairs, void *stream)
+{
+    int rc = splotch_render_host_async(ph, n, camera, cmh, params, out_rgb_host, workspace, workspace_bytes, max_pairs, stream);
+    if (rc) return rc;
+    int32_t status = SPLOTCH_OK;       // the status head sits at the start of the workspace in both layouts
+    rc = splotch_workspace_status(workspace, stream, &status, nullptr, nullptr);
+    return rc ? rc : status;
 }
 
 // ---------------------------------------------------------------------------------------------

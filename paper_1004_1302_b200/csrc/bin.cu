@@ -10,7 +10,6 @@ namespace splotch {
 namespace {
 
 constexpr int kBinThreads = 256;
-constexpr int kSmemBinsMax = 4096;          // two u32 arrays of this size live in shared memory
 
 struct BinBox {
     int x0, x1, y0, y1;
@@ -95,64 +94,166 @@ finish_offsets_kernel(const uint32_t *__restrict__ bin_count, const uint64_t *__
 }
 
 // ---------------------------------------------------------------------------------------------
-// scatter: list[bin_offset[b] + k] = particle index, any order inside a bin (additive mode).
-// A CTA takes a chunk of 1024 particles, counts its pairs per bin in shared memory, reserves
-// one range per touched bin with a single global atomic, then writes ids into the ranges.
+// scatter (a6): list[bin_offset[b] + k] = particle index, any order inside a bin (additive mode).
+// A CTA takes a chunk of 1024 consecutive particles (each warp 128 of them) and
+//   1. counts the chunk's pairs per bin with the difference-array trick of K1 (four shared atomics per
+//      splat, then a 2-D prefix sum over the (nbx + 1) x (nby + 1) grid in shared memory),
+//   2. reserves one range per touched bin with a single global atomic,
+//   3. enumerates the pairs DENSELY: every warp lays the boxes of its 128 splats end to end (warp scan of
+//      the box sizes) and lane l takes pairs l, l + 32, ...: owner by binary search in the 128 starts,
+//      bin by one reciprocal multiplication.  All 32 lanes work whatever the box sizes are (the first
+//      version let the owning lane walk small boxes and the warp walk big ones: 6 warp instructions per
+//      pair on C3, most of them idle lanes and integer divisions).
+// The packed bin boxes come from the compact array K1 writes beside the records (4 B per particle).
 // ---------------------------------------------------------------------------------------------
+constexpr int kScatWarps = kBinThreads / 32;
+constexpr int kScatPerLane = 4;                                  // splats per lane and chunk
+constexpr int kScatPerWarp = 32 * kScatPerLane;                  // 128
+constexpr int kScatChunk = kBinThreads * kScatPerLane;           // 1024
+constexpr int kScatDiffMax = 4608;                               // (nbx + 1)(nby + 1) entries in shared memory: up to 4096^2 images
+
+template <bool kSmem>
 __global__ void __launch_bounds__(kBinThreads)
-scatter_kernel(const void *__restrict__ records, int record_bytes, long long n, int nbx, int n_bins,
+scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby,
                const uint64_t *__restrict__ bin_offset, uint32_t *__restrict__ bin_cursor,
-               uint32_t *__restrict__ list, const WorkHead *head, int use_smem)
+               uint32_t *__restrict__ list, const WorkHead *head)
 {
     extern __shared__ uint32_t s_mem[];
     if (head->status != 0) return;
-    uint32_t *s_cnt = s_mem, *s_base = s_mem + n_bins;
-    constexpr int kPer = 4;
-    const long long chunk = (long long)kBinThreads * kPer;
-    const long long n_chunks = (n + chunk - 1) / chunk;
+    const int stride = nbx + 1, n_diff = kSmem ? stride * (nby + 1) : 0;
+    int *s_cnt = reinterpret_cast<int *>(s_mem);                 // difference grid -> counts -> running cursor of the chunk
+    uint32_t *s_base = s_mem + n_diff;                           // start of the chunk's range inside the bin's list
+    uint32_t *s_start = s_mem + 2 * n_diff;                      // [warp][129]: starts of the warp's boxes in its pair space
+    uint32_t *s_box = s_start + kScatWarps * (kScatPerWarp + 4); // [warp][128]: packed bin boxes
+    int *s_bb = reinterpret_cast<int *>(s_box + kScatWarps * kScatPerWarp);   // bounding box of the chunk on the grid
+    if (threadIdx.x == 0) { s_bb[0] = s_bb[1] = 1 << 20; s_bb[2] = s_bb[3] = -1; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *w_start = s_start + warp * (kScatPerWarp + 4), *w_box = s_box + warp * kScatPerWarp;
+    const long long n_chunks = (n + kScatChunk - 1) / kScatChunk;
     for (long long c = blockIdx.x; c < n_chunks; c += gridDim.x) {
-        uint32_t bins[kPer];
+        const long long first = c * kScatChunk + (long long)warp * kScatPerWarp;
+        uint32_t bins[kScatPerLane];
 #pragma unroll
-        for (int k = 0; k < kPer; ++k) {
-            const long long i = c * chunk + (long long)k * kBinThreads + threadIdx.x;
-            bins[k] = i < n ? record_bins(records, record_bytes, i) : kInvisible;
+        for (int k = 0; k < kScatPerLane; ++k) {
+            const long long i = first + k * 32 + lane;
+            bins[k] = i < n ? __ldg(binsw + i) : kInvisible;
         }
-        if (use_smem) {
-            for (int i = threadIdx.x; i < n_bins; i += kBinThreads) s_cnt[i] = 0u;
-            __syncthreads();
+        if (kSmem) {
+            // bounding box of the chunk's bin boxes: all sweeps below touch only that part of the grid (a chunk of
+            // spatially coherent particles covers a few bins of a 33 x 33 .. 65 x 65 grid)
+            int mnx = 1 << 20, mny = 1 << 20, mxx = -1, mxy = -1;
 #pragma unroll
-            for (int k = 0; k < kPer; ++k)
-                for_each_bin(bins[k], 0u, 0ull, nbx, [&](int b, int, uint32_t, unsigned long long) { atomicAdd(&s_cnt[b], 1u); });
+            for (int k = 0; k < kScatPerLane; ++k) {
+                if (bins[k] == kInvisible) continue;
+                const BinBox bb = unpack(bins[k]);
+                mnx = min(mnx, bb.x0); mny = min(mny, bb.y0); mxx = max(mxx, bb.x1 + 1); mxy = max(mxy, bb.y1 + 1);
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                mnx = min(mnx, __shfl_xor_sync(0xffffffffu, mnx, d)); mny = min(mny, __shfl_xor_sync(0xffffffffu, mny, d));
+                mxx = max(mxx, __shfl_xor_sync(0xffffffffu, mxx, d)); mxy = max(mxy, __shfl_xor_sync(0xffffffffu, mxy, d));
+            }
+            if (lane == 0 && mxx >= 0) {
+                atomicMin(&s_bb[0], mnx); atomicMin(&s_bb[1], mny); atomicMax(&s_bb[2], mxx); atomicMax(&s_bb[3], mxy);
+            }
             __syncthreads();
-            for (int i = threadIdx.x; i < n_bins; i += kBinThreads) {
-                const uint32_t cnt = s_cnt[i];
-                if (cnt) {
-                    s_base[i] = atomicAdd(&bin_cursor[i], cnt);
-                    s_cnt[i] = 0u;
+            const int rx0 = s_bb[0], ry0 = s_bb[1], rx1 = s_bb[2], ry1 = s_bb[3];     // grid region [rx0, rx1] x [ry0, ry1], inclusive
+            const int rw = rx1 - rx0 + 1, rn = rx1 >= rx0 ? rw * (ry1 - ry0 + 1) : 0;
+            for (int i = threadIdx.x; i < rn; i += kBinThreads) s_cnt[(ry0 + i / rw) * stride + rx0 + i % rw] = 0;
+            __syncthreads();
+            if (threadIdx.x == 0) { s_bb[0] = s_bb[1] = 1 << 20; s_bb[2] = s_bb[3] = -1; }    // for the next chunk
+#pragma unroll
+            for (int k = 0; k < kScatPerLane; ++k) {
+                if (bins[k] == kInvisible) continue;
+                const BinBox bb = unpack(bins[k]);
+                atomicAdd(&s_cnt[bb.y0 * stride + bb.x0], 1);
+                atomicAdd(&s_cnt[bb.y0 * stride + bb.x1 + 1], -1);
+                atomicAdd(&s_cnt[(bb.y1 + 1) * stride + bb.x0], -1);
+                atomicAdd(&s_cnt[(bb.y1 + 1) * stride + bb.x1 + 1], 1);
+            }
+            __syncthreads();
+            for (int y = ry0 + warp; y < ry1; y += kScatWarps) {    // prefix sums along x (row ry1 holds only closing impulses)
+                int carry = 0;
+                for (int x0 = rx0; x0 < rx1; x0 += 32) {
+                    const int x = x0 + lane;
+                    int v = x < rx1 ? s_cnt[y * stride + x] : 0;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const int u = __shfl_up_sync(0xffffffffu, v, d);
+                        if (lane >= d) v += u;
+                    }
+                    v += carry;
+                    if (x < rx1) s_cnt[y * stride + x] = v;
+                    carry = __shfl_sync(0xffffffffu, v, 31);
                 }
             }
             __syncthreads();
-#pragma unroll
-            for (int k = 0; k < kPer; ++k) {
-                const long long i = c * chunk + (long long)k * kBinThreads + threadIdx.x;
-                const uint32_t id = (uint32_t)i;
-                for_each_bin(bins[k], id, 0ull, nbx, [&](int b, int, uint32_t owner_id, unsigned long long) {
-                    const uint32_t pos = s_base[b] + atomicAdd(&s_cnt[b], 1u);
-                    list[bin_offset[b] + pos] = owner_id;
-                });
+            for (int x = rx0 + threadIdx.x; x < rx1; x += kBinThreads) {   // prefix sums along y
+                int run = 0;
+                for (int y = ry0; y < ry1; ++y) {
+                    run += s_cnt[y * stride + x];
+                    s_cnt[y * stride + x] = run;
+                }
             }
             __syncthreads();
-        } else {
-#pragma unroll
-            for (int k = 0; k < kPer; ++k) {
-                const long long i = c * chunk + (long long)k * kBinThreads + threadIdx.x;
-                const uint32_t id = (uint32_t)i;
-                for_each_bin(bins[k], id, 0ull, nbx, [&](int b, int, uint32_t owner_id, unsigned long long) {
-                    const uint32_t pos = atomicAdd(&bin_cursor[b], 1u);
-                    list[bin_offset[b] + pos] = owner_id;
-                });
+            for (int i = threadIdx.x; i < rn; i += kBinThreads) {
+                const int y = ry0 + i / rw, x = rx0 + i % rw;
+                const int cnt = (x < rx1 && y < ry1) ? s_cnt[y * stride + x] : 0;
+                if (cnt > 0) s_base[y * stride + x] = atomicAdd(&bin_cursor[y * nbx + x], (uint32_t)cnt);
+                s_cnt[y * stride + x] = 0;
             }
+            __syncthreads();
         }
+        // the warp's pair space: boxes of splat o = 32 k + lane laid end to end
+        uint32_t run = 0;
+#pragma unroll
+        for (int k = 0; k < kScatPerLane; ++k) {
+            const uint32_t cnt = bins[k] == kInvisible ? 0u : (uint32_t)unpack(bins[k]).count();
+            uint32_t inc = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += u;
+            }
+            w_start[k * 32 + lane] = run + inc - cnt;
+            w_box[k * 32 + lane] = bins[k];
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        const uint32_t total = run;
+        __syncwarp();
+        const bool aggregate = total <= 3u * kScatPerWarp;       // small boxes: neighbouring particles hit the same bins
+        for (uint32_t t0 = 0; t0 < total; t0 += 32) {            // warp-uniform trip count
+            const uint32_t t = t0 + lane;
+            const bool valid = t < total;
+            int lo = 0, hi = kScatPerWarp;                       // largest o with start[o] <= t (empty boxes share a start with their successor)
+#pragma unroll
+            for (int it = 0; it < 7; ++it) {
+                const int mid = (lo + hi) >> 1;
+                if (w_start[mid] <= t) lo = mid; else hi = mid;
+            }
+            const uint32_t local = valid ? t - w_start[lo] : 0u;
+            const BinBox bb = unpack(valid ? w_box[lo] : 0u);
+            const int cw = bb.width();
+            // local / cw: boxes have at most 256 x 256 bins, so (local + 1/2) / cw is at least 1/512 away from an integer
+            const int by = (int)(((float)local + 0.5f) * __frcp_rn((float)cw));
+            const int bx = bb.x0 + (int)local - by * cw, y = bb.y0 + by;
+            const uint32_t id = (uint32_t)(first + lo);
+            // lanes that hit the same bin in this step (small boxes of neighbouring particles) share one atomic and get
+            // consecutive positions, so their stores coalesce; big boxes give 32 different bins and singleton groups
+            const int key = valid ? y * stride + bx : -1 - lane;
+            const unsigned peers = aggregate ? __match_any_sync(0xffffffffu, key) : (1u << lane);
+            const int leader = __ffs(peers) - 1;
+            uint32_t base = 0;
+            if (valid && lane == leader) {
+                const uint32_t cnt = (uint32_t)__popc(peers);
+                if (kSmem) base = s_base[key] + (uint32_t)atomicAdd(&s_cnt[key], (int)cnt);
+                else base = atomicAdd(&bin_cursor[y * nbx + bx], cnt);
+            }
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (valid) list[__ldg(bin_offset + y * nbx + bx) + base + (uint32_t)__popc(peers & ((1u << lane) - 1u))] = id;
+        }
+        __syncthreads();
     }
 }
 
@@ -245,21 +346,25 @@ int launch_finish_offsets(const uint32_t *bin_count, const uint64_t *bin_offset,
     return 0;
 }
 
-int launch_scatter(const void *records, int record_bytes, int64_t n, const RenderConst &rc,
+int launch_scatter(const uint32_t *binsw, int64_t n, const RenderConst &rc,
                    const uint64_t *bin_offset, uint32_t *bin_cursor, uint32_t *list, uint64_t max_pairs,
                    const WorkHead *head, cudaStream_t st)
 {
     (void)max_pairs;
     if (n <= 0) return 0;
-    const int n_bins = rc.nbx * rc.nby;
-    const int use_smem = n_bins <= kSmemBinsMax ? 1 : 0;
-    const size_t smem = use_smem ? (size_t)n_bins * 2 * sizeof(uint32_t) : 0;
-    const long long chunk = (long long)kBinThreads * 4;
-    long long blocks = (n + chunk - 1) / chunk;
-    const long long cap = (long long)sm_count() * 6;
+    const int n_diff = (rc.nbx + 1) * (rc.nby + 1);
+    const bool use_smem = n_diff <= kScatDiffMax;
+    const size_t smem = ((use_smem ? 2 * (size_t)n_diff : 0) + kScatWarps * (kScatPerWarp + 4) + kScatWarps * kScatPerWarp + 4) *
+                        sizeof(uint32_t);
+    long long blocks = (n + kScatChunk - 1) / kScatChunk;
+    const long long cap = (long long)sm_count() * 8;
     if (blocks > cap) blocks = cap;
-    scatter_kernel<<<(unsigned)blocks, kBinThreads, smem, st>>>(records, record_bytes, (long long)n, rc.nbx, n_bins,
-                                                                bin_offset, bin_cursor, list, head, use_smem);
+    if (use_smem)
+        scatter_kernel<true><<<(unsigned)blocks, kBinThreads, smem, st>>>(binsw, (long long)n, rc.nbx, rc.nby, bin_offset,
+                                                                          bin_cursor, list, head);
+    else
+        scatter_kernel<false><<<(unsigned)blocks, kBinThreads, smem, st>>>(binsw, (long long)n, rc.nbx, rc.nby, bin_offset,
+                                                                           bin_cursor, list, head);
     SPLOTCH_LAUNCH_CHECK();
     return 0;
 }

@@ -161,14 +161,16 @@ int launch_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32
                       bool *result_in_tmp, const int32_t *status_dev = nullptr);
 
 // project.cu (K1): records + fused bin counts (+ optional debug outputs, + depth keys in absorb mode)
+// bin_diff: (nbx + 1) x (nby + 1) signed difference grid (zeroed by the caller), binsw: n packed bin boxes
 int launch_project(const ParticlePtrs &p, int64_t n, const CameraConst &cam, const RenderConst &rc,
-                   const float *lutE, const float *lutA, void *records, uint32_t *bin_count, uint32_t *zkeys,
+                   const float *lutE, const float *lutA, void *records, int *bin_diff, uint32_t *binsw, uint32_t *zkeys,
                    WorkHead *head, const DebugProjectOut *dbg, cudaStream_t st);
+int launch_bins_from_diff(int *bin_diff, const RenderConst &rc, uint32_t *bin_count, cudaStream_t st);
 
 // bin.cu (K2)
 int launch_finish_offsets(const uint32_t *bin_count, const uint64_t *bin_offset, int n_bins, uint64_t max_pairs,
                           uint32_t chunk, uint32_t *unit_prefix, WorkHead *head, cudaStream_t st);
-int launch_scatter(const void *records, int record_bytes, int64_t n, const RenderConst &rc,
+int launch_scatter(const uint32_t *binsw, int64_t n, const RenderConst &rc,
                    const uint64_t *bin_offset, uint32_t *bin_cursor, uint32_t *list, uint64_t max_pairs,
                    const WorkHead *head, cudaStream_t st);
 int launch_count_updates(const void *records, int record_bytes, int64_t n, const CameraConst &cam, float thr,

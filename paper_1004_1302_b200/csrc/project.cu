@@ -1,5 +1,5 @@
 // project.cu -- K1: fused transform / cull / colour kernel (steps a1-a3 of the hot path) with the
-// bin count (a4) folded in.
+// bin count (a4) folded in as a 2-D difference array.
 //
 // Reads the particle SoA (x, y, z, r, I, colval [, type]) with 128-bit coalesced loads, four
 // consecutive particles per thread, and writes one 32-byte (additive) or 48-byte (absorb) splat
@@ -14,7 +14,7 @@ namespace splotch {
 namespace {
 
 constexpr int kProjThreads = 256;
-constexpr int kSmemBinsMax = 8192;       // bins counted in shared memory when they fit
+constexpr int kSmemBinsMax = 8192;       // entries of the difference grid kept in shared memory when they fit
 constexpr float kSqrtPi = 1.7724538509055160273f;
 constexpr float kSqrtLog2e = 1.2011224087864498f;
 
@@ -81,46 +81,35 @@ __device__ __forceinline__ uint32_t pack_bins(const Projected &o, int shift)
            ((uint32_t)(o.j1 >> shift) << 24);
 }
 
-// Every bin of the splat's bin box gets one count (B-rules).  Small boxes are counted by the
-// owning lane, big ones by the whole warp so that one screen-filling splat does not stall 31 lanes.
-__device__ __forceinline__ void count_bins(uint32_t bins, uint32_t *hist, int nbx)
+// Bin counts (a4, B-rules: every bin of the splat's bin box gets one count) as a 2-D DIFFERENCE ARRAY: a box
+// (x0..x1) x (y0..y1) is four signed unit impulses at its corners on a (nbx + 1) x (nby + 1) grid, and the 2-D prefix
+// sum of the grid (bins_from_diff_kernel) is the count of every bin.  Four atomics per splat whatever the size of its
+// box (the first version walked the box: 9.4 atomics per splat on C3, and a screen-filling splat cost 1024).
+__device__ __forceinline__ void count_box(uint32_t bins, int *hist, int stride)
 {
-    const int lane = threadIdx.x & 31;
-    const bool vis = bins != kInvisible;
-    const int bx0 = bins & 255, bx1 = (bins >> 8) & 255, by0 = (bins >> 16) & 255, by1 = (bins >> 24) & 255;
-    const int w = bx1 - bx0 + 1, tot = w * (by1 - by0 + 1);
-    const bool big = vis && tot > 8;
-    if (vis && !big) {
-        for (int by = by0; by <= by1; ++by)
-            for (int bx = bx0; bx <= bx1; ++bx) atomicAdd(&hist[by * nbx + bx], 1u);
-    }
-    unsigned m = __ballot_sync(0xffffffffu, big);
-    while (m) {
-        const int src = __ffs(m) - 1;
-        m &= m - 1;
-        const uint32_t b = __shfl_sync(0xffffffffu, bins, src);
-        const int cx0 = b & 255, cx1 = (b >> 8) & 255, cy0 = (b >> 16) & 255, cy1 = (b >> 24) & 255;
-        const int cw = cx1 - cx0 + 1, ctot = cw * (cy1 - cy0 + 1);
-        for (int i = lane; i < ctot; i += 32) atomicAdd(&hist[(cy0 + i / cw) * nbx + cx0 + i % cw], 1u);
-    }
+    const int x0 = bins & 255, x1 = (bins >> 8) & 255, y0 = (bins >> 16) & 255, y1 = (bins >> 24) & 255;
+    atomicAdd(&hist[y0 * stride + x0], 1);
+    atomicAdd(&hist[y0 * stride + x1 + 1], -1);
+    atomicAdd(&hist[(y1 + 1) * stride + x0], -1);
+    atomicAdd(&hist[(y1 + 1) * stride + x1 + 1], 1);
 }
 
 template <bool kAbsorb>
 __global__ void __launch_bounds__(kProjThreads, 4)
 project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, const float *__restrict__ lutE,
-               const float *__restrict__ lutA, void *__restrict__ records, uint32_t *__restrict__ bin_count,
-               uint32_t *__restrict__ zkeys, WorkHead *head, DebugProjectOut dbg, int has_dbg, int vec_ok,
-               int smem_hist)
+               const float *__restrict__ lutA, void *__restrict__ records, int *__restrict__ bin_diff,
+               uint32_t *__restrict__ binsw, uint32_t *__restrict__ zkeys, WorkHead *head, DebugProjectOut dbg,
+               int has_dbg, int vec_ok, int smem_hist)
 {
-    extern __shared__ uint32_t s_hist[];
+    extern __shared__ int s_hist[];
     __shared__ unsigned int s_visible;
     __shared__ float s_area[2];
-    const int n_bins = rc.nbx * rc.nby;
+    const int diff_stride = rc.nbx + 1, n_diff = diff_stride * (rc.nby + 1);
     if (smem_hist)
-        for (int i = threadIdx.x; i < n_bins; i += blockDim.x) s_hist[i] = 0u;
+        for (int i = threadIdx.x; i < n_diff; i += blockDim.x) s_hist[i] = 0;
     if (threadIdx.x == 0) { s_visible = 0u; s_area[0] = s_area[1] = 0.0f; }
     __syncthreads();
-    uint32_t *hist = smem_hist ? s_hist : bin_count;
+    int *hist = smem_hist ? s_hist : bin_diff;
 
     unsigned int my_visible = 0;
     float my_area = 0.0f, my_tensor = 0.0f;     // heuristic for WorkHead::tensor_on, not part of the result
@@ -208,6 +197,7 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
                     rec[1] = make_float4(o.visible ? tau0 : 0.0f, er, eg, eb);
                     rec[2] = make_float4(ar, ag, ab, __uint_as_float(bins));
                 }
+                if (binsw) binsw[i] = bins;          // the packed bin box once more as a compact array: the scatter reads 4 B, not a 32-B record
                 if (zkeys) zkeys[i] = o.visible ? __float_as_uint(o.zc) : 0xFFFFFFFFu;
                 if (has_dbg) {
                     if (dbg.sx) dbg.sx[i] = o.sx;
@@ -221,7 +211,7 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
                     if (dbg.visible) dbg.visible[i] = o.visible ? 1 : 0;
                 }
             }
-            if (bin_count) count_bins(in ? bins : kInvisible, hist, rc.nbx);
+            if (bin_diff && in && o.visible) count_box(bins, hist, diff_stride);
         }
     }
     atomicAdd(&s_visible, my_visible);
@@ -231,10 +221,10 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
     }
     if ((threadIdx.x & 31) == 0) { atomicAdd(&s_area[0], my_area); atomicAdd(&s_area[1], my_tensor); }
     __syncthreads();
-    if (smem_hist && bin_count) {
-        for (int i = threadIdx.x; i < n_bins; i += blockDim.x) {
-            const uint32_t c = s_hist[i];
-            if (c) atomicAdd(&bin_count[i], c);
+    if (smem_hist && bin_diff) {
+        for (int i = threadIdx.x; i < n_diff; i += blockDim.x) {
+            const int c = s_hist[i];
+            if (c) atomicAdd(&bin_diff[i], c);
         }
     }
     if (threadIdx.x == 0 && s_visible) {
@@ -244,16 +234,54 @@ project_kernel(ParticlePtrs p, long long n, CameraConst cam, RenderConst rc, con
     }
 }
 
+// counts of all bins from the difference grid: prefix sums along x (one warp per grid row), then along y (one thread per
+// column).  One CTA: the grid has at most 257 x 257 entries and lives in L2.
+__global__ void __launch_bounds__(1024)
+bins_from_diff_kernel(int *__restrict__ diff, int nbx, int nby, uint32_t *__restrict__ bin_count)
+{
+    const int stride = nbx + 1, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int y = warp; y < nby; y += 32) {
+        int carry = 0;
+        for (int x0 = 0; x0 < nbx; x0 += 32) {
+            const int x = x0 + lane;
+            int v = x < nbx ? diff[y * stride + x] : 0;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, v, d);
+                if (lane >= d) v += u;
+            }
+            v += carry;
+            if (x < nbx) diff[y * stride + x] = v;
+            carry = __shfl_sync(0xffffffffu, v, 31);
+        }
+    }
+    __syncthreads();
+    for (int x = threadIdx.x; x < nbx; x += blockDim.x) {
+        int run = 0;
+        for (int y = 0; y < nby; ++y) {
+            run += diff[y * stride + x];
+            bin_count[y * nbx + x] = (uint32_t)run;
+        }
+    }
+}
+
 }  // namespace
 
+int launch_bins_from_diff(int *bin_diff, const RenderConst &rc, uint32_t *bin_count, cudaStream_t st)
+{
+    bins_from_diff_kernel<<<1, 1024, 0, st>>>(bin_diff, rc.nbx, rc.nby, bin_count);
+    SPLOTCH_LAUNCH_CHECK();
+    return 0;
+}
+
 int launch_project(const ParticlePtrs &p, int64_t n, const CameraConst &cam, const RenderConst &rc,
-                   const float *lutE, const float *lutA, void *records, uint32_t *bin_count, uint32_t *zkeys,
+                   const float *lutE, const float *lutA, void *records, int *bin_diff, uint32_t *binsw, uint32_t *zkeys,
                    WorkHead *head, const DebugProjectOut *dbg, cudaStream_t st)
 {
     if (n <= 0) return 0;
-    const int n_bins = rc.nbx * rc.nby;
-    const int smem_hist = (bin_count && n_bins <= kSmemBinsMax) ? 1 : 0;
-    const size_t smem = smem_hist ? (size_t)n_bins * sizeof(uint32_t) : 0;
+    const int n_diff = (rc.nbx + 1) * (rc.nby + 1);
+    const int smem_hist = (bin_diff && n_diff <= kSmemBinsMax) ? 1 : 0;
+    const size_t smem = smem_hist ? (size_t)n_diff * sizeof(int) : 0;
     auto aligned16 = [](const void *q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; };
     const int vec_ok = aligned16(p.x) && aligned16(p.y) && aligned16(p.z) && aligned16(p.r) && aligned16(p.I) &&
                        aligned16(p.colval) && (!p.type || (reinterpret_cast<uintptr_t>(p.type) & 3u) == 0);
@@ -265,11 +293,11 @@ int launch_project(const ParticlePtrs &p, int64_t n, const CameraConst &cam, con
     if (dbg) d = *dbg;
     if (rc.mode == 1)
         project_kernel<true><<<(unsigned)blocks, kProjThreads, smem, st>>>(p, (long long)n, cam, rc, lutE, lutA, records,
-                                                                           bin_count, zkeys, head, d, dbg ? 1 : 0,
+                                                                           bin_diff, binsw, zkeys, head, d, dbg ? 1 : 0,
                                                                            vec_ok, smem_hist);
     else
         project_kernel<false><<<(unsigned)blocks, kProjThreads, smem, st>>>(p, (long long)n, cam, rc, lutE, lutA, records,
-                                                                            bin_count, zkeys, head, d, dbg ? 1 : 0,
+                                                                            bin_diff, binsw, zkeys, head, d, dbg ? 1 : 0,
                                                                             vec_ok, smem_hist);
     SPLOTCH_LAUNCH_CHECK();
     return 0;

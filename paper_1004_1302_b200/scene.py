@@ -186,6 +186,42 @@ class Scene:
         B.splotch_render_host(ph, self.n, cs, cmh, ps, out_host, self._aligned(workspace), nbytes, max_pairs)
         return out_host, workspace
 
+    def render_host_pipelined(self, hb, n_frames: int, cam=None, mode: Optional[int] = None, max_pairs: Optional[int] = None,
+                              depth: int = 2):
+        """`n_frames` end-to-end frames (H2D of the inputs + render + D2H of the image, every frame) through
+        splotch_render_host_async with `depth` frames in flight: frame k + 1 is copied in while frame k is rasterised.
+        Each slot has its own stream, device workspace and pinned output image.  Returns the list of output images of
+        the last `depth` frames (pinned host tensors).  Synchronises at the end; raises if any frame failed."""
+        cam = cam or self.w.camera
+        cs, ps = _camera_struct(cam), self.params(mode)
+        max_pairs = self.max_pairs if max_pairs is None else max_pairs
+        ph = B.make_particles(hb["x"], hb["y"], hb["z"], hb["r"], hb["I"], hb["colval"], hb["type"])
+        cmh = B.make_colormap(hb["lut_e"], hb["lut_a"], self.n_entries, self.n_types)
+        nbytes = B.splotch_workspace_bytes_host(self.n, cs, cmh, ps, max_pairs)
+        if getattr(self, "_pipe", None) is None or self._pipe["nbytes"] != nbytes or len(self._pipe["ws"]) != depth:
+            self._pipe = dict(nbytes=nbytes, ws=[self._alloc(nbytes) for _ in range(depth)],
+                              streams=[torch.cuda.Stream(self.device) for _ in range(depth)],
+                              out=[torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory() for _ in range(depth)],
+                              busy=[False] * depth)
+        P = self._pipe
+
+        def finish(slot):
+            if P["busy"][slot]:
+                status, _, pairs = B.splotch_workspace_status(self._aligned(P["ws"][slot]), P["streams"][slot])
+                P["busy"][slot] = False
+                if status != B.SPLOTCH_OK:
+                    raise B.SplotchError(f"splotch_render_host_async (scene needs {pairs} pairs, max_pairs={max_pairs})", status)
+
+        for k in range(n_frames):
+            slot = k % depth
+            finish(slot)                      # the slot's previous frame has left its stream: its buffers are free again
+            B.splotch_render_host_async(ph, self.n, cs, cmh, ps, P["out"][slot], self._aligned(P["ws"][slot]), nbytes, max_pairs,
+                                        P["streams"][slot])
+            P["busy"][slot] = True
+        for slot in range(depth):
+            finish(slot)
+        return P["out"]
+
     def h2d_bytes(self) -> int:
         lut = self._host_lut_e.nbytes + (0 if self._host_lut_a is None else self._host_lut_a.nbytes)
         return self.n * (24 + (0 if self._host_type is None else 1)) + lut
