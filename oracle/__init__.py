@@ -17,7 +17,12 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "splotch_oracle.c")
-_LIB = os.path.join(_HERE, "libsplotch_oracle.so")
+# ORACLE_SANITIZE=1 builds a second library with AddressSanitizer + UndefinedBehaviorSanitizer;
+# run the pins under it with
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 ORACLE_SANITIZE=1 \
+#       python -m pytest tests/test_oracle_pins.py tests/test_oracle_canonical.py -q
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "libsplotch_oracle_asan.so" if _SANITIZE else "libsplotch_oracle.so")
 _lib = None
 
 ADDITIVE, ABSORB = 0, 1
@@ -27,7 +32,8 @@ def build(force: bool = False) -> str:
     """Compile the oracle.  -ffp-contract=off keeps the canonical fp32 sequence unfused."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".{os.getpid()}.tmp"
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared",
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all"] if _SANITIZE else ["-O2"]
+        cmd = ["gcc", *opt, "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared",
                "-fPIC", "-o", tmp, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)

@@ -222,36 +222,55 @@ scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby
         }
         const uint32_t total = run;
         __syncwarp();
-        const bool aggregate = total <= 3u * kScatPerWarp;       // small boxes: neighbouring particles hit the same bins
-        for (uint32_t t0 = 0; t0 < total; t0 += 32) {            // warp-uniform trip count
-            const uint32_t t = t0 + lane;
-            const bool valid = t < total;
-            int lo = 0, hi = kScatPerWarp;                       // largest o with start[o] <= t (empty boxes share a start with their successor)
+        // pair t of the warp: owner = largest o with start[o] <= t (empty boxes share a start with their successor), bin by
+        // one reciprocal multiplication: boxes have at most 256 x 256 bins, so (local + 1/2) / cw is at least 1/512 away
+        // from an integer and the approximate reciprocal (1 ulp) cannot move the quotient across one
+        auto locate = [&](uint32_t t, int &owner, int &bx, int &y) {
+            int lo = 0, hi = kScatPerWarp;
 #pragma unroll
             for (int it = 0; it < 7; ++it) {
                 const int mid = (lo + hi) >> 1;
                 if (w_start[mid] <= t) lo = mid; else hi = mid;
             }
-            const uint32_t local = valid ? t - w_start[lo] : 0u;
-            const BinBox bb = unpack(valid ? w_box[lo] : 0u);
+            const uint32_t local = t - w_start[lo];
+            const BinBox bb = unpack(w_box[lo]);
             const int cw = bb.width();
-            // local / cw: boxes have at most 256 x 256 bins, so (local + 1/2) / cw is at least 1/512 away from an integer
-            const int by = (int)(((float)local + 0.5f) * __frcp_rn((float)cw));
-            const int bx = bb.x0 + (int)local - by * cw, y = bb.y0 + by;
-            const uint32_t id = (uint32_t)(first + lo);
-            // lanes that hit the same bin in this step (small boxes of neighbouring particles) share one atomic and get
-            // consecutive positions, so their stores coalesce; big boxes give 32 different bins and singleton groups
-            const int key = valid ? y * stride + bx : -1 - lane;
-            const unsigned peers = aggregate ? __match_any_sync(0xffffffffu, key) : (1u << lane);
-            const int leader = __ffs(peers) - 1;
-            uint32_t base = 0;
-            if (valid && lane == leader) {
-                const uint32_t cnt = (uint32_t)__popc(peers);
-                if (kSmem) base = s_base[key] + (uint32_t)atomicAdd(&s_cnt[key], (int)cnt);
-                else base = atomicAdd(&bin_cursor[y * nbx + bx], cnt);
+            const int by = (int)(((float)local + 0.5f) * __fdividef(1.0f, (float)cw));
+            owner = lo;
+            bx = bb.x0 + (int)local - by * cw;
+            y = bb.y0 + by;
+        };
+        if (total > 3u * kScatPerWarp) {
+            // big boxes: the 32 pairs of a step lie in (mostly) different bins; one atomic and one store per pair
+            for (uint32_t t = lane; t < total; t += 32) {
+                int o, bx, y;
+                locate(t, o, bx, y);
+                uint32_t pos;
+                if (kSmem) pos = s_base[y * stride + bx] + (uint32_t)atomicAdd(&s_cnt[y * stride + bx], 1);
+                else pos = atomicAdd(&bin_cursor[y * nbx + bx], 1u);
+                list[__ldg(bin_offset + y * nbx + bx) + pos] = (uint32_t)(first + o);
             }
-            base = __shfl_sync(0xffffffffu, base, leader);
-            if (valid) list[__ldg(bin_offset + y * nbx + bx) + base + (uint32_t)__popc(peers & ((1u << lane) - 1u))] = id;
+        } else {
+            // small boxes: neighbouring particles hit the same bins; lanes with the same bin in a step share one atomic and
+            // get consecutive positions, so their stores coalesce
+            for (uint32_t t0 = 0; t0 < total; t0 += 32) {        // warp-uniform trip count
+                const uint32_t t = t0 + lane;
+                const bool valid = t < total;
+                int o = 0, bx = 0, y = 0;
+                if (valid) locate(t, o, bx, y);
+                const int key = valid ? y * stride + bx : -1 - lane;
+                const unsigned peers = __match_any_sync(0xffffffffu, key);
+                const int leader = __ffs(peers) - 1;
+                uint32_t base = 0;
+                if (valid && lane == leader) {
+                    const uint32_t cnt = (uint32_t)__popc(peers);
+                    if (kSmem) base = s_base[key] + (uint32_t)atomicAdd(&s_cnt[key], (int)cnt);
+                    else base = atomicAdd(&bin_cursor[y * nbx + bx], cnt);
+                }
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (valid)
+                    list[__ldg(bin_offset + y * nbx + bx) + base + (uint32_t)__popc(peers & ((1u << lane) - 1u))] = (uint32_t)(first + o);
+            }
         }
         __syncthreads();
     }

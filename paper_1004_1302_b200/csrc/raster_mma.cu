@@ -33,6 +33,8 @@
 //              inside a filter chunk, so the MMAs of batch b run while batch b + 1 is produced;
 //   flush    : tcgen05.ld of D, transposed through shared memory, vector red.global.add into the raw
 //              image (any summation order is legal when A = E).
+#include <type_traits>
+
 #include "raster_common.cuh"
 
 namespace splotch {
@@ -51,6 +53,12 @@ constexpr int kQueue = 1024;              // ring of admitted splats (power of t
 // ~2^-25 per MMA (measured on C3: -7e-5 with ~3700 MMAs per accumulator between flushes).  One unit of 4096 list
 // entries (~900 MMAs) keeps it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
 constexpr int kUnitsPerTicket = 1;
+// A batch whose 16 splats all have |a_c| <= kFaintAmp runs as ONE TF32 product per K step (operands rounded to nearest
+// TF32 by cvt.rna, no lo parts: a third of the MMAs, no operand split).  A single term is then off by at most
+// 2^-11 a_c w <= 3.8e-6 (4 % of the parity tolerance), and the roundings of different splats are independent and
+// zero-mean, so a pixel that sums N such terms is off by ~ 1.2e-4 sqrt(sum (a w)^2) <= 1.2e-4 sqrt(kFaintAmp S): 1.1e-5 at
+// S = 1 (all configs have a_c ~ 1e-5: ~4e-7).  Any brighter splat in the batch keeps the three-product split (2^-21 per term).
+constexpr float kFaintAmp = 0.0078125f;   // 2^-7
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
 constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
@@ -70,6 +78,7 @@ struct SmemMma {
         float stage[kBlockPx][kBlockPx * 3];                 // flush only
     };
     unsigned long long bar_full[2], bar_free[2];
+    uint32_t bright[kQueue / kMmaBatch];                     // per queued batch: some splat above kFaintAmp
     uint32_t tmem_base;
     uint32_t q_tail;
     uint32_t ticket;
@@ -144,6 +153,13 @@ __device__ __forceinline__ void queue_put(SmemMma &sm, uint32_t s, float sx, flo
 
 // v = hi + lo for both halves of a packed pair (Veltkamp split with 2^13 + 1: hi has 11 significant bits,
 // i.e. it is a TF32 number; lo = v - hi is exact; the tensor core ignores the 13 low bits of lo)
+__device__ __forceinline__ uint32_t round_tf32(float v)   // nearest TF32 (ties away): the tensor core would truncate
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
+    return r;
+}
+
 __device__ __forceinline__ void split_tf32x2(float2 v, float2 &hi, float2 &lo)
 {
     const float2 m1 = make_float2(-1.0f, -1.0f);
@@ -181,6 +197,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         asm volatile("fence.mbarrier_init.release.cluster;");
         sm.q_tail = 0;
     }
+    if (tid < kQueue / kMmaBatch) sm.bright[tid] = 0u;
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
@@ -207,8 +224,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     const uint64_t bdesc0 = b_descriptor(&sm.w.B[0][0][0][0]);
 
     // ---- nb batches of 16 queued splats; every role walks the same sequence ----
-    auto process_batches = [&](uint32_t nb) {
-        for (uint32_t it = 0; it < nb; ++it) {
+    // one batch, compiled twice: tag = true_type: three-product split; false_type: one product of rounded operands
+    auto one_batch = [&](auto tag) {
+        constexpr bool bright = decltype(tag)::value;
+        {
             const uint32_t buf = n_batches & 1u;
             const uint32_t uses = buf ? uses1 : uses0;
             if (warp == kIssuerWarp) {
@@ -222,11 +241,15 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                         const uint64_t b_hi = bdesc0 + (uint64_t)(((buf * 2 + g) * 2 + 0) * kBBytes >> 4);
                         const uint64_t b_lo = bdesc0 + (uint64_t)(((buf * 2 + g) * 2 + 1) * kBBytes >> 4);
                         mma_tf32_ts(d, a0, b_hi, kIdesc, fresh ? 0u : 1u);                 // K step 0: splats 0..7
-                        mma_tf32_ts(d, a0 + 16, b_hi, kIdesc, 1u);
-                        mma_tf32_ts(d, a0, b_lo, kIdesc, 1u);
+                        if (bright) {
+                            mma_tf32_ts(d, a0 + 16, b_hi, kIdesc, 1u);
+                            mma_tf32_ts(d, a0, b_lo, kIdesc, 1u);
+                        }
                         mma_tf32_ts(d, a0 + 8, b_hi + kStepUnits, kIdesc, 1u);             // K step 1: splats 8..15
-                        mma_tf32_ts(d, a0 + 24, b_hi + kStepUnits, kIdesc, 1u);
-                        mma_tf32_ts(d, a0 + 8, b_lo + kStepUnits, kIdesc, 1u);
+                        if (bright) {
+                            mma_tf32_ts(d, a0 + 24, b_hi + kStepUnits, kIdesc, 1u);
+                            mma_tf32_ts(d, a0 + 8, b_lo + kStepUnits, kIdesc, 1u);
+                        }
                     }
                     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
                                  ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
@@ -248,14 +271,18 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                         float2 t = __fmul2_rn(__fadd2_rn(xx, make_float2(q.x, q.y)), make_float2(q.z, q.w));
                         t = __fmul2_rn(t, t);
                         const float2 v = __fmul2_rn(qa[k], make_float2(ex2_approx(-t.x), ex2_approx(-t.y)));
-                        float2 h, l;
-                        split_tf32x2(v, h, l);
-                        hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
-                        lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
+                        if (bright) {
+                            float2 h, l;
+                            split_tf32x2(v, h, l);
+                            hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
+                            lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
+                        } else {
+                            hi[2 * k] = round_tf32(v.x);  hi[2 * k + 1] = round_tf32(v.y);
+                        }
                     }
                     const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
                     tmem_st16(a, hi);
-                    tmem_st16(a + 16, lo);
+                    if (bright) tmem_st16(a + 16, lo);
                     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                     asm volatile("tcgen05.fence::before_thread_sync;");
                 } else {
@@ -278,8 +305,9 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                             const float2 c0 = __fmul2_rn(make_float2(m.x, m.y), gy), c1 = __fmul2_rn(make_float2(m.z, m.w), gy);
                             const float2 f0 = make_float2(c0.x >= thr ? 1.0f : 0.0f, c0.y >= thr ? 1.0f : 0.0f);
                             const float2 f1 = make_float2(c1.x >= thr ? 1.0f : 0.0f, c1.y >= thr ? 1.0f : 0.0f);
-                            float2 h, l;
-                            split_tf32x2(gy, h, l);
+                            float2 h, l = make_float2(0.0f, 0.0f);
+                            if (bright) split_tf32x2(gy, h, l);
+                            else h = make_float2(__uint_as_float(round_tf32(gy.x)), __uint_as_float(round_tf32(gy.y)));
                             bh[0][k] = __fmul2_rn(h, f0);  bl[0][k] = __fmul2_rn(l, f0);
                             bh[1][k] = __fmul2_rn(h, f1);  bl[1][k] = __fmul2_rn(l, f1);
                         }
@@ -287,7 +315,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
 #pragma unroll
                         for (int g = 0; g < 2; ++g) {
                             *reinterpret_cast<float4 *>(&sm.w.B[buf][g][0][at]) = make_float4(bh[g][0].x, bh[g][0].y, bh[g][1].x, bh[g][1].y);
-                            *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0].x, bl[g][0].y, bl[g][1].x, bl[g][1].y);
+                            if (bright)
+                                *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0].x, bl[g][0].y, bl[g][1].x, bl[g][1].y);
                         }
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -299,6 +328,13 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
             n_batches += 1u;
             q_head += kMmaBatch;
             fresh = false;
+        }
+    };
+    auto process_batches = [&](uint32_t nb) {
+        for (uint32_t it = 0; it < nb; ++it) {
+            // the flag is set by the filter and stable while the batches run; the choice is uniform over the CTA
+            if (sm.bright[(q_head & (kQueue - 1)) / kMmaBatch] != 0u) one_batch(std::true_type{});
+            else one_batch(std::false_type{});
         }
     };
 
@@ -315,7 +351,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         }
         if (tid == 0) sm.q_tail = tail + pad;
         __syncthreads();
+        const uint32_t slot = (q_head & (kQueue - 1)) / kMmaBatch;
         process_batches(1u);
+        __syncthreads();                                  // every role has read the batch's flag
+        if (tid == 0) sm.bright[slot] = 0u;
     };
 
     // ---- wait for every MMA, add D to the raw image ----
@@ -448,13 +487,17 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                             const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
                             const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
                             queue_put(sm, s, g.x, g.y, g.z, amp.x, amp.y, amp.z, m0, m1);
+                            if (!(fmaxf(fmaxf(fabsf(amp.x), fabsf(amp.y)), fabsf(amp.z)) <= kFaintAmp)) atomicOr(&sm.bright[s / kMmaBatch], 1u);
                         }
                     }
                 }
                 __syncthreads();
                 const uint32_t tail = sm.q_tail;
+                const uint32_t head0 = q_head;
                 process_batches((tail - q_head) / kMmaBatch);
                 __syncthreads();                          // every warp is done reading the queue before it is refilled
+                for (uint32_t b = head0 / kMmaBatch + tid; b < q_head / kMmaBatch; b += kMmaThreads)
+                    sm.bright[b & (kQueue / kMmaBatch - 1)] = 0u;   // the filter sets flags of batches at or behind the tail only
             }
             drain();
             flush();

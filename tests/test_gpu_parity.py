@@ -252,6 +252,33 @@ def test_tensor_path_big_bright_splats(B, size):
     assert np.array_equal(outs[None], outs[True]) or np.allclose(outs[None], outs[False], rtol=1e-5, atol=1e-6)
 
 
+def test_tensor_path_mixed_bright_and_faint_splats(B):
+    """K3t runs a batch of 16 queued splats as ONE TF32 product when all of them are faint (|a_c| <= 2^-7) and as the
+    three-product split otherwise (raster_mma.cu: kFaintAmp).  Big splats, most of them faint (a ~ 1e-4 .. 5e-3), every 23rd
+    bright (a up to 0.3), so that both kinds of batches and mixed ones occur; a second scene holds faint splats only with
+    S of order 1, where a biased rounding of the operands (truncation instead of round-to-nearest) would show as a
+    relative offset of 2^-11 = 4.9e-4, five times the tolerance."""
+    rs = np.random.RandomState(17)
+    c = cam(eye=(0.0, 0.0, -10.0), fov=25.0, w=640, h=448)
+    for bright_every, n, amp_lo, amp_hi in ((23, 3000, 1e-4, 5e-3), (0, 8000, 2e-3, 7.5e-3)):
+        r = np.exp(rs.uniform(np.log(0.08), np.log(2.0), n))
+        amp = np.exp(rs.uniform(np.log(amp_lo), np.log(amp_hi), n))
+        if bright_every:
+            amp[::bright_every] = rs.uniform(0.05, 0.3, len(amp[::bright_every]))
+        pts = np.stack([rs.uniform(-3.2, 3.2, n), rs.uniform(-2.3, 2.3, n), rs.uniform(-1, 1, n), r,
+                        amp / (r * np.sqrt(np.pi)), rs.uniform(0.7, 1.0, n)], 1)
+        w = mk(pts, c, lut_e=const_lut((1.0, 0.7, 0.4)), support_f=3.1)
+        ref = oracle.render(w, raw=True)
+        assert ref.max() > 1.0
+        outs = {}
+        for tensor in (True, False):
+            outs[tensor] = _scene(w, tensor).render(raw=True).cpu().numpy()
+            _tol_check_masked(w, outs[tensor], ref, max_rim=0.25)
+        rel = (outs[True].astype(np.float64) - ref) / np.maximum(ref, 1e-30)
+        big = ref > 0.5
+        assert big.mean() > 0.2 and abs(float(rel[big].mean())) < 3e-5          # no systematic offset of the tensor path
+
+
 def test_absorb_scaled_c4(B):
     w = workloads.make("C4", 200_000, width=512, height=384)
     out, ref = _render_both(w)
