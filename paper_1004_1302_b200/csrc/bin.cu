@@ -159,8 +159,8 @@ scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby
             }
             __syncthreads();
             const int rx0 = s_bb[0], ry0 = s_bb[1], rx1 = s_bb[2], ry1 = s_bb[3];     // grid region [rx0, rx1] x [ry0, ry1], inclusive
-            const int rw = rx1 - rx0 + 1, rn = rx1 >= rx0 ? rw * (ry1 - ry0 + 1) : 0;
-            for (int i = threadIdx.x; i < rn; i += kBinThreads) s_cnt[(ry0 + i / rw) * stride + rx0 + i % rw] = 0;
+            for (int y = ry0 + warp; y <= ry1; y += kScatWarps)          // (an empty chunk has ry1 < ry0)
+                for (int x = rx0 + lane; x <= rx1; x += 32) s_cnt[y * stride + x] = 0;
             __syncthreads();
             if (threadIdx.x == 0) { s_bb[0] = s_bb[1] = 1 << 20; s_bb[2] = s_bb[3] = -1; }    // for the next chunk
 #pragma unroll
@@ -197,12 +197,12 @@ scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby
                 }
             }
             __syncthreads();
-            for (int i = threadIdx.x; i < rn; i += kBinThreads) {
-                const int y = ry0 + i / rw, x = rx0 + i % rw;
-                const int cnt = (x < rx1 && y < ry1) ? s_cnt[y * stride + x] : 0;
-                if (cnt > 0) s_base[y * stride + x] = atomicAdd(&bin_cursor[y * nbx + x], (uint32_t)cnt);
-                s_cnt[y * stride + x] = 0;
-            }
+            for (int y = ry0 + warp; y <= ry1; y += kScatWarps)
+                for (int x = rx0 + lane; x <= rx1; x += 32) {
+                    const int cnt = (x < rx1 && y < ry1) ? s_cnt[y * stride + x] : 0;
+                    if (cnt > 0) s_base[y * stride + x] = atomicAdd(&bin_cursor[y * nbx + x], (uint32_t)cnt);
+                    s_cnt[y * stride + x] = 0;
+                }
             __syncthreads();
         }
         // the warp's pair space: boxes of splat o = 32 k + lane laid end to end
@@ -242,13 +242,24 @@ scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby
         };
         if (total > 3u * kScatPerWarp) {
             // big boxes: the 32 pairs of a step lie in (mostly) different bins; one atomic and one store per pair
-            for (uint32_t t = lane; t < total; t += 32) {
-                int o, bx, y;
-                locate(t, o, bx, y);
+            auto emit = [&](int o, int bx, int y) {
                 uint32_t pos;
                 if (kSmem) pos = s_base[y * stride + bx] + (uint32_t)atomicAdd(&s_cnt[y * stride + bx], 1);
                 else pos = atomicAdd(&bin_cursor[y * nbx + bx], 1u);
                 list[__ldg(bin_offset + y * nbx + bx) + pos] = (uint32_t)(first + o);
+            };
+            uint32_t t = lane;
+            for (; t + 32 < total; t += 64) {                    // two pairs per lane and step: two independent search chains
+                int o0, bx0, y0, o1, bx1, y1;
+                locate(t, o0, bx0, y0);
+                locate(t + 32, o1, bx1, y1);
+                emit(o0, bx0, y0);
+                emit(o1, bx1, y1);
+            }
+            if (t < total) {
+                int o, bx, y;
+                locate(t, o, bx, y);
+                emit(o, bx, y);
             }
         } else {
             // small boxes: neighbouring particles hit the same bins; lanes with the same bin in a step share one atomic and

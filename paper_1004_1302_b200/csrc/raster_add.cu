@@ -192,7 +192,7 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                     full = seg_full(adm, g.y, g.z, thr, py0, m0, m1);
                 }
             }
-            unsigned hb0 = 0u, hb1 = 0u;            // bit k: row part + 8k handled in segment 0 / 1
+            unsigned hbits = 0u;                    // bit 2k + g: row part + 8k handled in segment g
             const float yb = pixel_centre(py0 + part);
             const float2 thr2 = make_float2(thr, thr), scale2 = make_float2(kMaskScale, kMaskScale);
 #pragma unroll
@@ -208,36 +208,32 @@ raster_additive_kernel(const SplatAdd *__restrict__ records, const uint32_t *__r
                     const float2 c0 = __fmul2_rn(make_float2(m0, m0), gy), c1 = __fmul2_rn(make_float2(m1, m1), gy);
                     hd0 = adm & (full | (c0.x >= thr ? 1u : 0u) | (c1.x >= thr ? 2u : 0u));
                     hd1 = adm & (full | (c0.y >= thr ? 1u : 0u) | (c1.y >= thr ? 2u : 0u));
+                    hbits |= (hd0 | (hd1 << 2)) << (2 * k);
                 }
-                hb0 |= ((hd0 & 1u) << k) | ((hd1 & 1u) << (k + 1));
-                hb1 |= ((hd0 >> 1) << k) | ((hd1 >> 1) << (k + 1));
-                const uint32_t w0 = (__float_as_uint(Wm.x) & 0x7ffffffeu) | ((hd0 & 1u) << 31) | (hd0 >> 1);
-                const uint32_t w1 = (__float_as_uint(Wm.y) & 0x7ffffffeu) | ((hd1 & 1u) << 31) | (hd1 >> 1);
+                const uint32_t w0 = (__float_as_uint(Wm.x) & 0x7ffffffeu) | (hd0 << 31) | (hd0 >> 1);
+                const uint32_t w1 = (__float_as_uint(Wm.y) & 0x7ffffffeu) | (hd1 << 31) | (hd1 >> 1);
                 const float2 wr = __fmul2_rn(make_float2(a.x, a.x), gy), wg = __fmul2_rn(make_float2(a.y, a.y), gy);
                 const float2 wb = __fmul2_rn(make_float2(a.z, a.z), gy);
                 sm.row[slot][s][part + 8 * k] = make_float4(wr.x, wg.x, wb.x, __uint_as_float(w0));
                 sm.row[slot][s][part + 8 * k + 8] = make_float4(wr.y, wg.y, wb.y, __uint_as_float(w1));
             }
-            unsigned all0 = hb0, all1 = hb1, any0 = hb0, any1 = hb1;
+            // over the 8 threads of the splat, in one word: low half = handled in SOME thread's row, high half = NOT handled in some
+            unsigned red = hbits | ((~hbits & 0xffffu) << 16);
             if (mma_on) {
 #pragma unroll
-                for (int d = 1; d < 8; d <<= 1) {
-                    all0 &= __shfl_xor_sync(0xffffffffu, all0, d);
-                    all1 &= __shfl_xor_sync(0xffffffffu, all1, d);
-                    any0 |= __shfl_xor_sync(0xffffffffu, any0, d);
-                    any1 |= __shfl_xor_sync(0xffffffffu, any1, d);
-                }
+                for (int d = 1; d < 8; d <<= 1) red |= __shfl_xor_sync(0xffffffffu, red, d);
             }
+            const unsigned any_h = red & 0xffffu, not_all = red >> 16;
             unsigned short c2 = 0;
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 const int t = 2 * part + k;
                 const int tpx = px0 + (t & 3) * kTilePx, tpy = py0 + (t >> 2) * kTilePx;
                 int cl = valid ? classify_tile(g.x, g.y, g.w, (float)tpx + 0.5f, (float)tpy + 0.5f, W, H, tpx, tpy) : 0;
-                const unsigned rows2 = 3u << (2 * (t >> 2));           // the tile's 16 rows are bits 2ty, 2ty+1 of every part
-                const unsigned all = (t & 2) ? all1 : all0, any = (t & 2) ? any1 : any0;
-                if ((all & rows2) == rows2) cl = 0;                    // every row of the tile is done on the tensor cores
-                else if ((any & rows2) && cl == 2) cl = 1;             // some rows are: take the masking path
+                // the tile's 16 rows are rows k = 2 ty, 2 ty + 1 of every thread; its segment is g = (t >> 1) & 1
+                const unsigned rows2 = (5u << ((t >> 1) & 1)) << (4 * (t >> 2));
+                if (mma_on && (not_all & rows2) == 0u) cl = 0;         // every row of the tile is done on the tensor cores
+                else if ((any_h & rows2) && cl == 2) cl = 1;           // some rows are: take the masking path
                 c2 |= (unsigned short)(cl << (8 * k));
             }
             *reinterpret_cast<unsigned short *>(&sm.cls[slot][s][2 * part]) = c2;
