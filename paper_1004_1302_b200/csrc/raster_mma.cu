@@ -111,6 +111,13 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
                  : "memory");
 }
 
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+}
+
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
@@ -153,12 +160,9 @@ __device__ __forceinline__ void queue_put(SmemMma &sm, uint32_t s, float sx, flo
 
 // v = hi + lo for both halves of a packed pair (Veltkamp split with 2^13 + 1: hi has 11 significant bits,
 // i.e. it is a TF32 number; lo = v - hi is exact; the tensor core ignores the 13 low bits of lo)
-__device__ __forceinline__ uint32_t round_tf32(float v)   // nearest TF32 (ties away): the tensor core would truncate
-{
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
-    return r;
-}
+// nearest TF32 (ties away) of a finite value well inside the fp32 range: add half a TF32 ulp to the bit pattern; the
+// tensor core ignores the 13 low bits.  (cvt.rna.tf32.f32 does the same plus an inf/nan test, two instructions.)
+__device__ __forceinline__ uint32_t round_tf32(float v) { return __float_as_uint(v) + 0x1000u; }
 
 __device__ __forceinline__ void split_tf32x2(float2 v, float2 &hi, float2 &lo)
 {
@@ -226,7 +230,9 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     // ---- nb batches of 16 queued splats; every role walks the same sequence ----
     // one batch, compiled twice: tag = true_type: three-product split; false_type: one product of rounded operands
     auto one_batch = [&](auto tag) {
-        constexpr bool bright = decltype(tag)::value;
+        constexpr int mode = decltype(tag)::value;           // 0: 16 faint splats, 1: 16 splats split, 2: 32 faint splats
+        constexpr bool bright = mode == 1;
+        constexpr int n_splats = mode == 2 ? 2 * kMmaBatch : kMmaBatch;
         {
             const uint32_t buf = n_batches & 1u;
             const uint32_t uses = buf ? uses1 : uses0;
@@ -250,6 +256,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                             mma_tf32_ts(d, a0 + 24, b_hi + kStepUnits, kIdesc, 1u);
                             mma_tf32_ts(d, a0 + 8, b_lo + kStepUnits, kIdesc, 1u);
                         }
+                        if (mode == 2) {                                                   // splats 16..31 sit where the lo parts would
+                            mma_tf32_ts(d, a0 + 16, b_hi + 2 * kStepUnits, kIdesc, 1u);
+                            mma_tf32_ts(d, a0 + 24, b_hi + 3 * kStepUnits, kIdesc, 1u);
+                        }
                     }
                     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
                                  ::"r"(smem_u32(&sm.bar_free[buf])) : "memory");
@@ -264,25 +274,31 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                     const uint32_t qp = (q_head & (kQueue - 1)) >> 1;              // a batch never wraps: 16 | kQueue
                     const float4 *qg = &sm.w.qG[qp];
                     const float2 *qa = &sm.w.qAmp[quarter][qp];
-                    uint32_t hi[16], lo[16];
-#pragma unroll
-                    for (int k = 0; k < kMmaBatch / 2; ++k) {                      // two splats per step, f32x2 arithmetic
-                        const float4 q = qg[k];
-                        float2 t = __fmul2_rn(__fadd2_rn(xx, make_float2(q.x, q.y)), make_float2(q.z, q.w));
-                        t = __fmul2_rn(t, t);
-                        const float2 v = __fmul2_rn(qa[k], make_float2(ex2_approx(-t.x), ex2_approx(-t.y)));
-                        if (bright) {
-                            float2 h, l;
-                            split_tf32x2(v, h, l);
-                            hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
-                            lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
-                        } else {
-                            hi[2 * k] = round_tf32(v.x);  hi[2 * k + 1] = round_tf32(v.y);
-                        }
-                    }
+                    // Every channel warp evaluates the column exponentials itself.  Sharing them through shared memory (the
+                    // channel-0 warp computes, a named barrier, the other two read) removes two thirds of the MUFU work but
+                    // puts the three warps in series: measured K3t 96 -> 105 ms on C3; the batch pipeline is latency-bound.
                     const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
-                    tmem_st16(a, hi);
-                    if (bright) tmem_st16(a + 16, lo);
+#pragma unroll
+                    for (int half = 0; half < n_splats / 8; ++half) {              // 8 splats at a time: two splats per step, f32x2 arithmetic
+                        uint32_t hi[8], lo[8];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const float4 q = qg[4 * half + k];
+                            float2 t = __fmul2_rn(__fadd2_rn(xx, make_float2(q.x, q.y)), make_float2(q.z, q.w));
+                            t = __fmul2_rn(t, t);
+                            const float2 v = __fmul2_rn(qa[4 * half + k], make_float2(ex2_approx(-t.x), ex2_approx(-t.y)));
+                            if (bright) {
+                                float2 h, l;
+                                split_tf32x2(v, h, l);
+                                hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
+                                lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
+                            } else {
+                                hi[2 * k] = round_tf32(v.x);  hi[2 * k + 1] = round_tf32(v.y);
+                            }
+                        }
+                        tmem_st8(a + 8 * half, hi);                                // faint splats 16..31 land in the columns of the lo parts
+                        if (bright) tmem_st8(a + 16 + 8 * half, lo);
+                    }
                     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                     asm volatile("tcgen05.fence::before_thread_sync;");
                 } else {
@@ -292,8 +308,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                     const uint32_t qp = (q_head & (kQueue - 1)) >> 1;
                     const float4 *qg = &sm.w.qBg[qp], *qm = &sm.w.qBm[qp];
 #pragma unroll
-                    for (int qq = 0; qq < 2; ++qq) {
-                        const int q4 = 2 * b_half + qq;                           // group of 4 splats = 2 pairs
+                    for (int qq = 0; qq < n_splats / 8; ++qq) {
+                        const int q4 = 2 * b_half + (qq & 1) + 4 * (qq >> 1);     // group of 4 splats = 2 pairs; this warp's 8 of every 16
                         float2 bh[2][2], bl[2][2];                                // [group][pair]
 #pragma unroll
                         for (int k = 0; k < 2; ++k) {
@@ -314,9 +330,10 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                         const int at = (q4 * kBlockPx + j) * 4;
 #pragma unroll
                         for (int g = 0; g < 2; ++g) {
-                            *reinterpret_cast<float4 *>(&sm.w.B[buf][g][0][at]) = make_float4(bh[g][0].x, bh[g][0].y, bh[g][1].x, bh[g][1].y);
+                            float *Bg = &sm.w.B[buf][g][0][0];             // hi operand, then the lo operand (or faint splats 16..31)
+                            *reinterpret_cast<float4 *>(Bg + at) = make_float4(bh[g][0].x, bh[g][0].y, bh[g][1].x, bh[g][1].y);
                             if (bright)
-                                *reinterpret_cast<float4 *>(&sm.w.B[buf][g][1][at]) = make_float4(bl[g][0].x, bl[g][0].y, bl[g][1].x, bl[g][1].y);
+                                *reinterpret_cast<float4 *>(Bg + kMmaBatch * kBlockPx + at) = make_float4(bl[g][0].x, bl[g][0].y, bl[g][1].x, bl[g][1].y);
                         }
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -326,15 +343,24 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
             }
             if (buf) uses1 += 1u; else uses0 += 1u;
             n_batches += 1u;
-            q_head += kMmaBatch;
+            q_head += n_splats;
             fresh = false;
         }
     };
     auto process_batches = [&](uint32_t nb) {
-        for (uint32_t it = 0; it < nb; ++it) {
-            // the flag is set by the filter and stable while the batches run; the choice is uniform over the CTA
-            if (sm.bright[(q_head & (kQueue - 1)) / kMmaBatch] != 0u) one_batch(std::true_type{});
-            else one_batch(std::false_type{});
+        for (uint32_t it = 0; it < nb;) {
+            // the flags are set by the filter and stable while the batches run; the choice is uniform over the CTA
+            const uint32_t at = q_head & (kQueue - 1);
+            if (sm.bright[at / kMmaBatch] != 0u) {
+                one_batch(std::integral_constant<int, 1>{});
+                it += 1;
+            } else if (it + 1 < nb && at + 2 * kMmaBatch <= kQueue && sm.bright[at / kMmaBatch + 1] == 0u) {
+                one_batch(std::integral_constant<int, 2>{});      // two faint batches as one: half the hand-offs per splat
+                it += 2;
+            } else {
+                one_batch(std::integral_constant<int, 0>{});
+                it += 1;
+            }
         }
     };
 
