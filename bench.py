@@ -300,7 +300,9 @@ def main():
                            unit="TFLOP/s", frac=t_achieved / tf32_peak, traffic=read_traffic(w.name, "raster_additive_mma_kernel"),
                            kernel_ms=tensor_ms, kernel_share_of_step=tensor_ms / ms_frame, updates_per_launch=upd_tensor,
                            algorithmic_flops_per_update=6.0,
-                           executed_over_algorithmic=4.0,   # 3 split-TF32 products x 128/96 padded accumulator rows
+                           # 128/96 padded accumulator rows x the TF32 products per term: 1 for a batch of faint splats
+                           # (|a_c| <= 2^-7: every splat of C1..C5), 3 (split operands) for a batch with a brighter one
+                           executed_over_algorithmic="1.33 (faint batches) .. 4.0 (three-product split)",
                            peak_source=f"0.5 x sustained dense BF16 cuBLAS throughput ({peaks['source']}) = TF32 dense")
     # the dominant kernel by time is the headline roofline; the whole rasteriser is also quoted in ALU terms
     roofline = alu_roof if (not tensor_used or alu_ms >= tensor_ms) else tensor_roof

@@ -70,8 +70,9 @@ typedef struct {
     /* Optional vector colouring ("the three components of the vectors can be mapped to the three
      * components of E and A"; reading R19): when vr is not NULL, vr / vg / vb (length n, all three required) give
      * E_p = brightness[type] * (vr, vg, vb) and A_p = abs_brightness[type] * (vr, vg, vb) directly, used as given
-     * (no clamp); colval and the colour tables are ignored (colval may then be NULL); a particle with a non-finite
-     * component is culled.  Zero-initialise the struct to keep the scalar path. */
+     * (no clamp); colval and the colour tables are ignored (colval and the table pointers of splotch_colormap may then be
+     * NULL; n_types is still read); a particle with a non-finite component is culled.  Zero-initialise the struct to keep
+     * the scalar path. */
     const float *vr, *vg, *vb;
 } splotch_particles;
 

@@ -124,10 +124,13 @@ int make_render_const(const splotch_camera *cam, const splotch_colormap *cm, con
     return SPLOTCH_OK;
 }
 
-int check_colormap(const splotch_colormap *cm, int mode)
+// vector colouring (reading R19) ignores the tables: they may then be NULL (the struct still carries n_types)
+int check_colormap(const splotch_colormap *cm, int mode, bool vector_colouring = false)
 {
-    if (!cm || !cm->emission) return SPLOTCH_ERR_INVALID_ARG;
-    if (cm->n_entries < 2 || cm->n_types < 1 || cm->n_types > SPLOTCH_MAX_TYPES) return SPLOTCH_ERR_INVALID_ARG;
+    if (!cm) return SPLOTCH_ERR_INVALID_ARG;
+    if (cm->n_types < 1 || cm->n_types > SPLOTCH_MAX_TYPES) return SPLOTCH_ERR_INVALID_ARG;
+    if (vector_colouring) return SPLOTCH_OK;
+    if (!cm->emission || cm->n_entries < 2) return SPLOTCH_ERR_INVALID_ARG;
     if (mode == SPLOTCH_ABSORB && !cm->absorption) return SPLOTCH_ERR_INVALID_ARG;
     return SPLOTCH_OK;
 }
@@ -224,7 +227,7 @@ int setup(const splotch_particles *particles, int64_t n, const splotch_camera *c
     rc = make_camera(camera, &c->cam);
     if (rc) return rc;
     if (!params) return SPLOTCH_ERR_INVALID_ARG;
-    rc = check_colormap(cm, params->mode);
+    rc = check_colormap(cm, params->mode, n > 0 && particles && particles->vr);
     if (rc) return rc;
     rc = make_render_const(camera, cm, params, bin_shift, &c->rc);
     if (rc) return rc;

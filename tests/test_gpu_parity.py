@@ -576,3 +576,10 @@ def test_vector_colouring_matches_oracle(B, mode):
     w.lut_e = w.lut_e[:, ::-1].copy()
     out2 = _scene(w).render(raw=(mode == ADDITIVE)).cpu().numpy()
     np.testing.assert_allclose(out2, out, rtol=2e-5, atol=1e-6)
+    # ... and may be absent altogether (include/splotch.h: the table pointers may be NULL with vector colouring)
+    sc3 = _scene(w)
+    sc3.d["colval"] = None
+    sc3.d["lut_e"] = None
+    sc3.d["lut_a"] = None
+    out3 = sc3.render(raw=(mode == ADDITIVE)).cpu().numpy()
+    np.testing.assert_allclose(out3, out, rtol=2e-5, atol=1e-6)
