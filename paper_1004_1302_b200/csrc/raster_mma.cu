@@ -18,7 +18,8 @@
 // v = hi + lo with hi a TF32 number (Veltkamp split with 2^13 + 1 in packed f32x2 arithmetic: hi has 11
 // significant bits, lo = v - hi exactly; the tensor core ignores the 13 low bits of lo), and three
 // products are accumulated (hi*hi + lo*hi + hi*lo), which leaves a relative error of ~2^-21 per term
-// instead of 2^-11 -- fp32 class, inside the 1e-4 parity tolerance for any amplitude.
+// instead of 2^-11 -- fp32 class, inside the 1e-4 parity tolerance for any amplitude.  A batch of
+// splats that are all faint (|a_c| <= kFaintAmp, see below) needs one product of rounded operands.
 //
 // One CTA (11 warps, 2 CTAs per SM, 256 of the 512 TMEM columns each) owns a block for up to
 // kUnitsPerTicket consecutive work units of its splat list:
@@ -26,9 +27,10 @@
 //              seg_admit() and appends admitted splats to a ring queue in shared memory; entries whose
 //              block is missed by the circle or entirely handled here get kListDone set in the list,
 //              so the ALU kernel (which runs next) drops them without fetching the record;
-//   batch    : 16 queued splats.  Warps 0-2 / 4-6 (channel = warp & 3, group = warp >> 2) produce A into
-//              tensor memory, warps 3, 7, 8, 9 produce B (32 block rows x 8 splats each), warp 10 issues
-//              the 12 MMAs of the batch.  Two buffers; producers -> issuer through an mbarrier `full`,
+//   batch    : 16 queued splats (32 when two consecutive faint batches are available).  Warps 0-2 / 4-6
+//              (channel = warp & 3, group = warp >> 2) produce A into tensor memory, warps 3, 7, 8, 9 produce
+//              B (32 block rows x 8 of every 16 splats each), warp 10 issues the MMAs of the batch (12 with
+//              split operands, 4 or 8 for faint batches).  Two buffers; producers -> issuer through an mbarrier `full`,
 //              issuer -> producers through tcgen05.commit on an mbarrier `free`; no CTA-wide barrier
 //              inside a filter chunk, so the MMAs of batch b run while batch b + 1 is produced;
 //   flush    : tcgen05.ld of D, transposed through shared memory, vector red.global.add into the raw
@@ -54,7 +56,7 @@ constexpr int kQueue = 1024;              // ring of admitted splats (power of t
 // entries (~900 MMAs) keeps it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
 constexpr int kUnitsPerTicket = 1;
 // A batch whose 16 splats all have |a_c| <= kFaintAmp runs as ONE TF32 product per K step (operands rounded to nearest
-// TF32 by cvt.rna, no lo parts: a third of the MMAs, no operand split).  A single term is then off by at most
+// TF32, no lo parts: a third of the MMAs, no operand split).  A single term is then off by at most
 // 2^-11 a_c w <= 3.8e-6 (4 % of the parity tolerance), and the roundings of different splats are independent and
 // zero-mean, so a pixel that sums N such terms is off by ~ 1.2e-4 sqrt(sum (a w)^2) <= 1.2e-4 sqrt(kFaintAmp S): 1.1e-5 at
 // S = 1 (all configs have a_c ~ 1e-5: ~4e-7).  Any brighter splat in the batch keeps the three-product split (2^-21 per term).
