@@ -74,3 +74,25 @@ def test_compute_entry_points_need_a_device(lib):
     from paper_1004_1302_b200 import Scene
     with pytest.raises(RuntimeError):
         Scene(workloads.make("C1", 100))
+
+
+def test_bench_reference_arm_prints_one_json_line():
+    """bench.py --impl reference is the CPU oracle on the box's host cores (no GPU needed): one JSON line with the
+    contract's keys; under torchrun every rank but 0 exits without work."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--workload", "C1", "--steps", "1", "--warmup", "0"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env={**os.environ, "RANK": "0", "WORLD_SIZE": "1"})
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "Mparticles/s" and d["value"] > 0 and d["higher_is_better"] is True
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
+    assert "C1" in d["config"]["workload"]
+    out1 = subprocess.run(cmd, capture_output=True, text=True, timeout=120, env={**os.environ, "RANK": "1", "WORLD_SIZE": "2"})
+    assert out1.returncode == 0 and out1.stdout.strip() == ""
