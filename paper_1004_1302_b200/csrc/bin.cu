@@ -228,7 +228,7 @@ scatter_kernel(const uint32_t *__restrict__ binsw, long long n, int nbx, int nby
         auto locate = [&](uint32_t t, int &owner, int &bx, int &y) {
             int lo = 0, hi = kScatPerWarp;
 #pragma unroll
-            for (int it = 0; it < 7; ++it) {
+            for (int it = 0; (1 << it) < kScatPerWarp; ++it) {
                 const int mid = (lo + hi) >> 1;
                 if (w_start[mid] <= t) lo = mid; else hi = mid;
             }
