@@ -29,7 +29,9 @@
  *   - Asynchrony: splotch_render, splotch_normalize and the debug calls only enqueue work on
  *     `stream` (a cudaStream_t passed as void*, NULL = default stream) and return without
  *     synchronising.  Calls whose name ends in _sync or that return host values synchronise
- *     the stream; they say so below.
+ *     the stream; they say so below.  splotch_render and splotch_render_batch issue only
+ *     memsets and kernel launches on `stream`, so they can be captured into a CUDA graph
+ *     and replayed over the same buffers (tests/test_gpu_parity.py does).
  *   - Image layout: out_rgb[(row * width + col) * 3 + c], float32, row 0 = top of the image,
  *     c = 0,1,2 = R,G,B.  Pixel (col i, row j) is sampled at its centre (i + 1/2, j + 1/2).
  *   - Errors: 0 = SPLOTCH_OK, negative = error, nothing is ever reported through the image.

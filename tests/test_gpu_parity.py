@@ -471,6 +471,40 @@ def test_render_batch_orbit_matches_oracle_per_camera(B):
                            sc.workspace.numel() - 256, sc.max_pairs)
 
 
+def test_render_is_capturable_in_a_cuda_graph(B):
+    """splotch_render only enqueues on the caller's stream (include/splotch.h "Asynchrony"): it can be captured into a CUDA
+    graph and replayed, in both modes; the replayed image equals the eagerly rendered one (ALU paths are deterministic up to
+    the order of atomics) and a replay after the particle arrays changed in place renders the new scene."""
+    for name, kw in (("C1", dict(n=30_000, width=160, height=128)), ("C4", dict(n=20_000, width=160, height=128))):
+        w = workloads.make(name, **kw)
+        sc = _scene(w, tensor=False)
+        sc.reserve()
+        cam_ = w.camera
+        out = torch.zeros((cam_.height, cam_.width, 3), dtype=torch.float32, device="cuda")
+        eager = sc.render(out=out.clone()).cpu().numpy()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            sc.render(out=out, check=False)                    # warm-up on the capture stream
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            sc.render(out=out, check=False)
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(out.cpu().numpy(), eager, rtol=2e-5, atol=1e-6)
+        status, _, _ = B.splotch_workspace_status(sc._aligned(sc.workspace))
+        assert status == B.SPLOTCH_OK
+        sc.d["I"].mul_(0.5)                                     # same buffers, new content: the graph renders the new scene
+        graph.replay()
+        torch.cuda.synchronize()
+        w.I = w.I * np.float32(0.5)
+        ref = oracle.render(w)
+        _tol_check(out.cpu().numpy(), ref, f"{name} graph replay")
+
+
 def test_stats_counts(B):
     w = workloads.make("C1")
     sc = _scene(w)
