@@ -535,6 +535,30 @@ def test_render_host_matches_device_render(B):
     _tol_check(out_host.numpy(), ref, "render_host")
 
 
+def test_render_host_async_pipelined_frames(B):
+    """splotch_render_host_async: frames streamed with two in flight (two streams, two workspaces).  Every frame must
+    equal the synchronous call; changing a host array between frames changes exactly the frames enqueued afterwards; a
+    frame whose pair capacity is too small reports it through the status head of its own workspace."""
+    w = workloads.make("C3", 150_000, width=256, height=192)
+    sc = _scene(w)
+    sc.reserve()
+    hb = sc.host_buffers()
+    ref_host, _ = sc.render_host(hb)
+    ref_host = ref_host.numpy().copy()
+    outs = sc.render_host_pipelined(hb, 5)                     # frames 3 and 4 are in the two slots at the end
+    for o in outs:
+        np.testing.assert_allclose(o.numpy(), ref_host, rtol=2e-5, atol=1e-6)
+    _tol_check(outs[0].numpy(), oracle.render(w), "pipelined host render")
+    hb["I"].mul_(0.5)                                          # pinned host array changed in place: the next frames see it
+    outs = sc.render_host_pipelined(hb, 2)
+    w.I = w.I * np.float32(0.5)
+    ref2 = oracle.render(w)
+    for o in outs:
+        _tol_check(o.numpy(), ref2, "pipelined host render, changed input")
+    with pytest.raises(B.SplotchError):
+        sc.render_host_pipelined(hb, 2, max_pairs=sc.max_pairs // 4)
+
+
 # ------------------------------------------------------------------------------------------------
 # stage (b): range normalisation of a scalar field on the device
 # ------------------------------------------------------------------------------------------------
