@@ -282,6 +282,39 @@ uint64_t splotch_sort_scratch_bytes(int64_t n);
 int splotch_debug_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, int64_t n,
                              int32_t key_bits, void *scratch, uint64_t scratch_bytes, void *stream);
 
+/* ------------------------------------------------------------------------------------------
+ * splotch_scan_static: the bin-offset scan (step a5, bin counts -> bin offsets) with NO caller-supplied
+ * scratch and NO allocation of any kind.
+ *
+ * Who needs it.  A renderer of this kind can be run "in situ": linked into the simulation that produces the
+ * particles and called between its time steps.  Such a host program has normally handed all of the GPU's memory
+ * to its own pool at start-up and forbids its plug-ins to call cudaMalloc: the call could fail, or succeed and make the
+ * simulation's next step run out of memory, and cudaMalloc / cudaFree stall every stream of the device while
+ * they run, the simulation's included.  A caller in that position has device buffers for its data (the counts
+ * and the offsets) but nothing to spare for the scan's tile descriptors, and cannot get any.  For it, the
+ * descriptors live in a fixed 66,048-byte __device__ array that is part of the library image.
+ *
+ *   in   DEVICE, n uint32 (may be NULL when n == 0)        out  DEVICE, n + 1 uint64, caller-owned
+ *   out[k] = in[0] + ... + in[k-1] for k = 0..n (out[n] = total), the same values splotch_debug_scan writes.
+ *
+ * Limit: n <= SPLOTCH_SCAN_STATIC_MAX_N (2^24 counts; a 16384 x 16384 image has 65,536 production bins and
+ *   1,048,576 16x16 tiles).  A larger n returns SPLOTCH_ERR_LIMIT and enqueues nothing; use splotch_debug_scan
+ *   with your own scratch instead.
+ * Cost: every GPU on which this library is loaded holds the 66,048 bytes until the process exits, used or not.
+ * Allocation: the call issues one memset and one kernel on `stream` (enqueue only, no synchronisation).  It
+ *   calls no cudaMalloc, cudaFree, or any library routine that allocates.
+ * First call on a device: looks up that device's address of the array (cudaGetSymbolAddress, with the calling
+ *   thread's current device) and keeps it for later calls.  Make this first call during set-up, with the right
+ *   device current and before any stream capture is begun.
+ * Sharing: there is one array per device and every call uses it.  The call clears the part it needs before the
+ *   kernel runs, so earlier contents never matter; but two calls that can overlap on the GPU (different streams
+ *   without an ordering between them, or two host threads on one device) corrupt each other's descriptors and
+ *   may hang.  Calls on one stream, or ordered by events, are safe.
+ * Errors: SPLOTCH_ERR_INVALID_ARG (n < 0, NULL out, NULL in with n > 0), SPLOTCH_ERR_LIMIT, SPLOTCH_ERR_CUDA.
+ * ---------------------------------------------------------------------------------------- */
+#define SPLOTCH_SCAN_STATIC_MAX_N (1 << 24)
+int splotch_scan_static(const uint32_t *in, uint64_t *out, int64_t n, void *stream);
+
 /* Per-stage timing of splotch_render with CUDA events recorded on the caller's stream (used by
  * bench.py for the roofline of the dominant kernel).  splotch_profile_enable(1) resets the
  * record; while enabled every splotch_render records 7 events (up to 256 calls).

@@ -33,6 +33,7 @@ EXPORTS = [
     "splotch_workspace_bytes", "splotch_render", "splotch_render_batch", "splotch_workspace_status", "splotch_count_pairs",
     "splotch_normalize", "splotch_field_range", "splotch_field_normalize", "splotch_tonemap_rgb8", "splotch_workspace_bytes_host", "splotch_render_host", "splotch_render_host_async", "splotch_debug_project",
     "splotch_debug_bins", "splotch_debug_workspace_bytes", "splotch_debug_stats", "splotch_debug_tensor_stats", "splotch_debug_scan",
+    "splotch_scan_static",
     "splotch_sort_scratch_bytes", "splotch_debug_sort_pairs", "splotch_status_string",
     "splotch_last_cuda_error", "splotch_version", "splotch_profile_enable", "splotch_profile_read",
     "splotch_launch_count",
@@ -311,6 +312,19 @@ def splotch_debug_scan(inp, out, n: int, scratch, scratch_bytes: int, stream=Non
     _check("splotch_debug_scan", _lib().splotch_debug_scan(_vp(_ptr(inp)), _vp(_ptr(out)), C.c_int64(n),
                                                            _vp(_ptr(scratch)), C.c_uint64(scratch_bytes),
                                                            _vp(_stream(stream))))
+
+
+SPLOTCH_SCAN_STATIC_MAX_N = 1 << 24
+
+
+def splotch_scan_static(inp, out, n: int, stream=None) -> None:
+    """Exclusive scan of n uint32 counts into n + 1 uint64 offsets, like splotch_debug_scan, for callers that cannot
+    give the library scratch memory and are not allowed to allocate any (a renderer embedded in a simulation whose own
+    pool holds all of the GPU's memory): the scan's bookkeeping sits in a fixed 66,048-byte array inside the library.
+    n <= SPLOTCH_SCAN_STATIC_MAX_N, else SplotchError(SPLOTCH_ERR_LIMIT).  Calls on one device share that array: keep
+    them on one stream or order them.  Marshalling only; see include/splotch.h."""
+    _check("splotch_scan_static", _lib().splotch_scan_static(_vp(_ptr(inp)), _vp(_ptr(out)), C.c_int64(n),
+                                                             _vp(_stream(stream))))
 
 
 def splotch_sort_scratch_bytes(n: int) -> int:

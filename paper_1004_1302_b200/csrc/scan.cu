@@ -7,6 +7,7 @@
 // prefix.  A descriptor is one 64-bit word: status in the top two bits, value below, so one
 // store publishes both.
 #include "common.cuh"
+#include "splotch.h"
 
 namespace splotch {
 
@@ -146,4 +147,54 @@ int launch_scan_u32_u32(const uint32_t *in, uint32_t *out, int64_t n, void *scra
     return launch_scan<uint32_t>(in, out, n, scratch, st);
 }
 
+// ---------------------------------------------------------------------------------------------
+// splotch_scan_static: the same scan for callers that have no device memory to hand over as scratch and may not
+// ask the CUDA allocator for any (include/splotch.h says who they are).  The ticket and the tile descriptors live
+// in the array below, which is part of the library image: every GPU that loads the library carries these
+// 66,048 bytes until the process exits, whether the entry point is ever called or not.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int64_t kStaticScanMaxN = 1 << 24;                                  // = SPLOTCH_SCAN_STATIC_MAX_N
+constexpr int64_t kStaticScanTiles = kStaticScanMaxN / kScanTile;             // 8192
+constexpr size_t kStaticScanBytes = (256 + (kStaticScanTiles + 1) * 8 + 255) / 256 * 256;   // same layout as launch_scan
+
+static __device__ __align__(256) unsigned char g_static_scan_scratch[kStaticScanBytes];
+
+// On the host the name g_static_scan_scratch is only a handle for the runtime, not a device address; the address
+// differs per device and has to be asked for with that device current.  Looked up once per device and kept.
+std::atomic<void *> g_static_scan_ptr[kMaxDevices];
+
+int static_scan_scratch(void **out)
+{
+    int dev = -1;
+    SPLOTCH_CUDA_TRY(cudaGetDevice(&dev));
+    const bool slot = dev >= 0 && dev < kMaxDevices;
+    void *p = slot ? g_static_scan_ptr[dev].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        SPLOTCH_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scan_scratch));
+        if (!p) return -3;
+        if (slot) g_static_scan_ptr[dev].store(p, std::memory_order_release);   // racing threads store the same value
+    }
+    *out = p;
+    return 0;
+}
+
+}  // namespace
+
 }  // namespace splotch
+
+extern "C" int splotch_scan_static(const uint32_t *in, uint64_t *out, int64_t n, void *stream)
+{
+    using namespace splotch;
+    static_assert(kStaticScanMaxN == SPLOTCH_SCAN_STATIC_MAX_N, "header and kernel file disagree on the limit");
+    static_assert(kStaticScanBytes == 66048, "the size the header and README quote");
+    if (n < 0 || !out || (n > 0 && !in)) return SPLOTCH_ERR_INVALID_ARG;
+    if (n > kStaticScanMaxN) return SPLOTCH_ERR_LIMIT;      // the descriptor array has no room for more tiles
+    void *scratch = nullptr;
+    const int rc = static_scan_scratch(&scratch);
+    if (rc) return rc;
+    // launch_scan zeroes the ticket and the descriptors it is about to use (a memset enqueued on the stream, not an
+    // allocation), so what the previous call left in the array does not matter.
+    return launch_scan_u32_u64(in, out, n, scratch, reinterpret_cast<cudaStream_t>(stream));
+}
