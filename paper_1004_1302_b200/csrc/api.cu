@@ -179,7 +179,7 @@ Layout make_layout(int64_t n, int nbx, int nby, int mode, uint64_t max_pairs, bo
     L.records = take(nn * (mode == SPLOTCH_ABSORB ? sizeof(SplatAbs) : sizeof(SplatAdd)));
     L.bin_diff_bytes = (uint64_t)(nbx + 1) * (uint64_t)(nby + 1) * 4;
     L.bin_diff = take(L.bin_diff_bytes);
-    L.binsw = take(nn * 4);
+    if (mode != SPLOTCH_ABSORB) L.binsw = take(nn * 4);      // read by the additive scatter only; absorb lists come from the records
     L.bin_count = take((uint64_t)n_bins * 4);
     L.bin_cursor = take((uint64_t)n_bins * 4);
     L.bin_offset = take((uint64_t)(n_bins + 1) * 8);
@@ -253,7 +253,7 @@ int run_front(const Ctx &c, const splotch_particles *particles, int64_t n, const
     if (n > 0) pp = { particles->x, particles->y, particles->z, particles->r, particles->I, particles->colval, particles->type,
                       particles->vr, particles->vg, particles->vb };
     int rc = launch_project(pp, n, c.cam, c.rc, cm->emission, cm->absorption, c.ws + c.L.records,
-                            c.at<int>(c.L.bin_diff), c.at<uint32_t>(c.L.binsw),
+                            c.at<int>(c.L.bin_diff), c.rc.mode == SPLOTCH_ABSORB ? nullptr : c.at<uint32_t>(c.L.binsw),
                             c.rc.mode == SPLOTCH_ABSORB ? c.at<uint32_t>(c.L.zkeys) : nullptr, c.head(), dbg, c.st);
     if (rc) return rc;
     rc = launch_bins_from_diff(c.at<int>(c.L.bin_diff), c.rc, c.at<uint32_t>(c.L.bin_count), c.st);

@@ -51,6 +51,10 @@ constexpr int kFilterThreads = 256;       // warps 0-7 filter
 constexpr int kPerThread = 2;             // list entries per filter thread and pass
 constexpr int kFilterChunk = kFilterThreads * kPerThread;   // list entries per filter pass
 constexpr int kQueue = 1024;              // ring of admitted splats (power of two, > kFilterChunk + a batch)
+// Ring of per-batch "bright" flags, indexed by the unwrapped batch number: TWICE the queue's batch count, so that the
+// flags a filter pass sets (batches from the tail on, at most kFilterChunk + kMmaBatch - 1 entries ahead) can never be
+// the ones the previous pass's consumed batches are still being cleared from (no barrier separates the two).
+constexpr int kFlagRing = 2 * kQueue / kMmaBatch;
 // The tensor core adds every K = 8 dot product into the fp32 accumulator with truncation: a relative deficit of
 // ~2^-25 per MMA (measured on C3: -7e-5 with ~3700 MMAs per accumulator between flushes).  One unit of 4096 list
 // entries (~900 MMAs) keeps it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
@@ -80,7 +84,7 @@ struct SmemMma {
         float stage[kBlockPx][kBlockPx * 3];                 // flush only
     };
     unsigned long long bar_full[2], bar_free[2];
-    uint32_t bright[kQueue / kMmaBatch];                     // per queued batch: some splat above kFaintAmp
+    uint32_t bright[kFlagRing];                              // per queued batch: some splat above kFaintAmp (or not finite)
     uint32_t tmem_base;
     uint32_t q_tail;
     uint32_t ticket;
@@ -186,7 +190,6 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int quarter = warp & 3, grp = (warp >> 2) & 1;   // TMEM lane quarter (= channel for quarter < 3), column group
     const bool a_warp = warp < 8 && quarter < 3;
-    const bool b_warp = (warp < 8 && quarter == 3) || warp == 8 || warp == 9;
     const int b_rows = warp == 3 ? 0 : warp == 7 ? 1 : warp == 8 ? 0 : 1;     // which 32 block rows
     const int b_half = warp < 8 ? 0 : 1;                                      // which 8 splats of the batch
     const uint32_t n_units = head->n_units;
@@ -203,7 +206,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         asm volatile("fence.mbarrier_init.release.cluster;");
         sm.q_tail = 0;
     }
-    if (tid < kQueue / kMmaBatch) sm.bright[tid] = 0u;
+    if (tid < kFlagRing) sm.bright[tid] = 0u;
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
@@ -352,11 +355,11 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
     auto process_batches = [&](uint32_t nb) {
         for (uint32_t it = 0; it < nb;) {
             // the flags are set by the filter and stable while the batches run; the choice is uniform over the CTA
-            const uint32_t at = q_head & (kQueue - 1);
-            if (sm.bright[at / kMmaBatch] != 0u) {
+            const uint32_t at = q_head & (kQueue - 1), fb = q_head / kMmaBatch;
+            if (sm.bright[fb & (kFlagRing - 1)] != 0u) {
                 one_batch(std::integral_constant<int, 1>{});
                 it += 1;
-            } else if (it + 1 < nb && at + 2 * kMmaBatch <= kQueue && sm.bright[at / kMmaBatch + 1] == 0u) {
+            } else if (it + 1 < nb && at + 2 * kMmaBatch <= kQueue && sm.bright[(fb + 1) & (kFlagRing - 1)] == 0u) {
                 one_batch(std::integral_constant<int, 2>{});      // two faint batches as one: half the hand-offs per splat
                 it += 2;
             } else {
@@ -379,7 +382,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         }
         if (tid == 0) sm.q_tail = tail + pad;
         __syncthreads();
-        const uint32_t slot = (q_head & (kQueue - 1)) / kMmaBatch;
+        const uint32_t slot = (q_head / kMmaBatch) & (kFlagRing - 1);
         process_batches(1u);
         __syncthreads();                                  // every role has read the batch's flag
         if (tid == 0) sm.bright[slot] = 0u;
@@ -512,10 +515,14 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                         if (lane == 0 && bal) base = atomicAdd(&sm.q_tail, (uint32_t)__popc(bal));
                         base = __shfl_sync(0xffffffffu, base, 0);
                         if (adm) {
-                            const uint32_t s = (base + __popc(bal & ((1u << lane) - 1u))) & (kQueue - 1);
+                            const uint32_t pos = base + __popc(bal & ((1u << lane) - 1u));   // unwrapped queue position
+                            const uint32_t s = pos & (kQueue - 1);
                             const float4 amp = __ldg(reinterpret_cast<const float4 *>(records + id) + 1);
                             queue_put(sm, s, g.x, g.y, g.z, amp.x, amp.y, amp.z, m0, m1);
-                            if (!(fmaxf(fmaxf(fabsf(amp.x), fabsf(amp.y)), fabsf(amp.z)) <= kFaintAmp)) atomicOr(&sm.bright[s / kMmaBatch], 1u);
+                            // written so that a NaN amplitude counts as bright (fmaxf would drop it): the split path carries
+                            // non-finite values through like the ALU kernel, the integer TF32 rounding does not
+                            if (!(fabsf(amp.x) <= kFaintAmp && fabsf(amp.y) <= kFaintAmp && fabsf(amp.z) <= kFaintAmp))
+                                atomicOr(&sm.bright[(pos / kMmaBatch) & (kFlagRing - 1)], 1u);
                         }
                     }
                 }
@@ -525,7 +532,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                 process_batches((tail - q_head) / kMmaBatch);
                 __syncthreads();                          // every warp is done reading the queue before it is refilled
                 for (uint32_t b = head0 / kMmaBatch + tid; b < q_head / kMmaBatch; b += kMmaThreads)
-                    sm.bright[b & (kQueue / kMmaBatch - 1)] = 0u;   // the filter sets flags of batches at or behind the tail only
+                    sm.bright[b & (kFlagRing - 1)] = 0u;    // the next pass sets flags from the tail on: other slots (kFlagRing)
             }
             drain();
             flush();
