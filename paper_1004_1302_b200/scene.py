@@ -41,6 +41,7 @@ class Scene:
         self.d = {}
         self.workspace: Optional[torch.Tensor] = None
         self.max_pairs = 0
+        self._counted = set()     # (camera, mode) keys whose pair count render_batch has already checked against max_pairs
         self.tensor = None        # additive mode: None = library decides, True = SPLOTCH_FORCE_TENSOR, False = SPLOTCH_NO_TENSOR
         if resident:
             self.upload()
@@ -70,6 +71,10 @@ class Scene:
 
     def _alloc(self, nbytes: int) -> torch.Tensor:
         return torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=self.device)
+
+    def _cam_key(self, cam, mode):
+        return (tuple(cam.eye), tuple(cam.lookat), tuple(cam.up), float(cam.fov_deg), int(cam.width), int(cam.height),
+                self.w.mode if mode is None else mode)
 
     @staticmethod
     def _aligned(t: torch.Tensor) -> int:
@@ -126,9 +131,17 @@ class Scene:
         K = len(cams)
         cs = [_camera_struct(c) for c in cams]
         ps = self.params(mode, raw)
-        if self.workspace is None or self.max_pairs == 0:
-            worst = max(self.count_pairs(c, mode)[0] for c in cams) if K else 0
-            self.reserve(cams[0] if K else None, mode, max_pairs=worst + 1024)
+        # A workspace reserved earlier for ONE camera may be too small for another camera of the batch: the pair counts of
+        # cameras this scene has not counted yet are taken once (synchronising) and the workspace grown if one needs more.
+        # Cameras already counted cost nothing, so a steady orbit loop, or a caller that lowers max_pairs on purpose, is
+        # left alone.
+        new = [c for c in cams if self._cam_key(c, mode) not in self._counted]
+        if new or self.workspace is None:
+            worst = max(self.count_pairs(c, mode)[0] for c in new) if new else 0
+            self._counted.update(self._cam_key(c, mode) for c in new)
+            need = B.splotch_workspace_bytes(self.n, cs[0], ps, max(self.max_pairs, worst)) if K else 0
+            if self.workspace is None or self.max_pairs < worst or self.workspace.numel() < need + 256:
+                self.reserve(cams[0] if K else None, mode, max_pairs=max(self.max_pairs, worst + 1024))
         H, W = (cams[0].height, cams[0].width) if K else (0, 0)
         if out is None:
             out = torch.empty((K, H, W, 3), dtype=torch.float32, device=self.device)
@@ -198,8 +211,10 @@ class Scene:
         ph = B.make_particles(hb["x"], hb["y"], hb["z"], hb["r"], hb["I"], hb["colval"], hb["type"])
         cmh = B.make_colormap(hb["lut_e"], hb["lut_a"], self.n_entries, self.n_types)
         nbytes = B.splotch_workspace_bytes_host(self.n, cs, cmh, ps, max_pairs)
-        if getattr(self, "_pipe", None) is None or self._pipe["nbytes"] != nbytes or len(self._pipe["ws"]) != depth:
-            self._pipe = dict(nbytes=nbytes, ws=[self._alloc(nbytes) for _ in range(depth)],
+        # keyed on the image shape too: a camera with width and height swapped needs the same bytes but another (H, W)
+        key = (cam.height, cam.width, nbytes, depth)
+        if getattr(self, "_pipe", None) is None or self._pipe["key"] != key:
+            self._pipe = dict(key=key, nbytes=nbytes, ws=[self._alloc(nbytes) for _ in range(depth)],
                               streams=[torch.cuda.Stream(self.device) for _ in range(depth)],
                               out=[torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory() for _ in range(depth)],
                               busy=[False] * depth)

@@ -505,6 +505,102 @@ def test_render_is_capturable_in_a_cuda_graph(B):
         _tol_check(out.cpu().numpy(), ref, f"{name} graph replay")
 
 
+def test_tensor_path_and_batch_are_capturable_in_a_cuda_graph(B):
+    """The header's capture claim also covers the tensor-core rasteriser and splotch_render_batch: a forced-tensor render
+    and a two-camera batch, captured and replayed, give the eagerly rendered images (sums may be reordered: within rounding)
+    and match the oracle."""
+    import dataclasses
+    w = workloads.make("C3", 60_000, width=256, height=192)
+    cam2 = dataclasses.replace(w.camera, fov_deg=w.camera.fov_deg * 0.8)
+    sc = _scene(w, tensor=True)
+    sc.reserve(max_pairs=max(sc.count_pairs(c)[0] for c in (w.camera, cam2)) + 1024)
+    H, W = w.camera.height, w.camera.width
+    side = torch.cuda.Stream()
+
+    def capture(fn):
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            fn()                                               # warm-up on the capture stream
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            fn()
+        return graph
+
+    out = torch.zeros((H, W, 3), dtype=torch.float32, device="cuda")
+    eager = sc.render(raw=True).cpu().numpy()
+    assert sc.tensor_stats()[0] > 0                            # the tensor-core kernel really has work in this scene
+    g1 = capture(lambda: sc.render(raw=True, out=out, check=False))
+    out.zero_()
+    g1.replay()
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(out.cpu().numpy(), eager, rtol=2e-5, atol=1e-6)
+    _tol_check(out.cpu().numpy(), oracle.render(w, raw=True), "tensor path, graph replay")
+
+    outs = torch.zeros((2, H, W, 3), dtype=torch.float32, device="cuda")
+    eager2, _ = sc.render_batch([w.camera, cam2], raw=True)
+    eager2 = eager2.cpu().numpy()
+    g2 = capture(lambda: sc.render_batch([w.camera, cam2], raw=True, out=outs, check=False))
+    outs.zero_()
+    g2.replay()
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(outs.cpu().numpy(), eager2, rtol=2e-5, atol=1e-6)
+    _tol_check(outs[1].cpu().numpy(), oracle.render(w, camera=cam2, raw=True), "batch frame 1, graph replay")
+
+
+def test_nan_amplitude_is_not_dropped_by_the_tensor_path(B):
+    """A colour table with a NaN entry gives some splats a NaN amplitude.  The ALU rasteriser carries it into every pixel
+    such a splat covers; the tensor-core rasteriser must not turn it into a number (its faint single-product path rounds
+    bit patterns, which would): every pixel that is NaN on the ALU path is NaN with the tensor cores forced on."""
+    rs = np.random.RandomState(5)
+    n = 400
+    pts = np.stack([rs.uniform(-1.2, 1.2, n), rs.uniform(-1.2, 1.2, n), rs.uniform(-0.5, 0.5, n), rs.uniform(0.3, 0.5, n),
+                    np.full(n, 1e-3), rs.uniform(0, 1, n)], 1)
+    lut = np.linspace(0.2, 1.0, 8 * 3, dtype=np.float32).reshape(8, 3)
+    lut[5, 1] = np.nan
+    w = mk(pts, cam(w=256, h=192), lut_e=lut)
+    imgs = {}
+    for tensor in (False, True):
+        sc = _scene(w, tensor=tensor)
+        imgs[tensor] = sc.render(raw=True).cpu().numpy()
+        if tensor:
+            assert sc.tensor_stats()[0] > 0
+    nan_alu, nan_tc = np.isnan(imgs[False]), np.isnan(imgs[True])
+    assert nan_alu.any() and not nan_alu[..., 0].any()          # only the green channel holds the NaN entry
+    assert (nan_tc | ~nan_alu).all()
+    both = ~nan_alu & ~nan_tc
+    np.testing.assert_allclose(imgs[True][both], imgs[False][both], rtol=2e-4, atol=1e-6)
+
+
+def test_scene_caches_follow_the_camera(B):
+    """Scene.render_batch grows a workspace that was reserved for a camera with fewer pairs instead of failing, and the
+    pinned output images of render_host_pipelined are re-made when width and height swap (same byte count)."""
+    import dataclasses
+    w = workloads.make("C5", 100_000, width=160, height=128)
+    sc = _scene(w, tensor=False)
+    pairs = [sc.count_pairs(c)[0] for c in w.cameras]
+    small = w.cameras[int(np.argmin(pairs))]
+    assert max(pairs) > min(pairs)
+    sc.reserve(small, slack=1.0)
+    sc.max_pairs = min(pairs)                                   # exactly what the smallest camera needs
+    imgs, status = sc.render_batch(raw=True)                    # would raise without the re-reserve
+    assert (status.cpu().numpy()[:, 0] == 0).all() and sc.max_pairs >= max(pairs)
+    k = int(np.argmax(pairs))
+    _tol_check(imgs[k].cpu().numpy(), oracle.render(w, camera=w.cameras[k], raw=True), "batch after growing the workspace")
+
+    w2 = workloads.make("C3", 50_000, width=192, height=128)
+    sc2 = _scene(w2)
+    tall = dataclasses.replace(w2.camera, width=128, height=192)
+    sc2.reserve(max_pairs=max(sc2.count_pairs(c)[0] for c in (w2.camera, tall)) + 1024)
+    hb = sc2.host_buffers()
+    a = sc2.render_host_pipelined(hb, 2)[0]
+    assert tuple(a.shape) == (128, 192, 3)
+    b = sc2.render_host_pipelined(hb, 2, cam=tall)[0]
+    assert tuple(b.shape) == (192, 128, 3)
+    _tol_check(b.numpy(), oracle.render(w2, camera=tall), "pipelined host render, transposed image shape")
+
+
 def test_stats_counts(B):
     w = workloads.make("C1")
     sc = _scene(w)
