@@ -34,6 +34,7 @@ import numpy as np  # noqa: E402
 METRIC = "Mparticles/s rendered and achieved HBM GB/s fraction on one B200"
 SM_COUNT_NOMINAL = 148
 LANES_PER_SM = 128
+L2_BYTES = 126 * 1000 * 1000                 # B200 L2 (B200_PROFILING.md)
 ALGO_LANE_OPS_PER_UPDATE = {0: 5.0, 1: 17.0}   # 1 mul + 3 FMA + 1 test; absorb adds 3 exp + ~9 ops
 
 
@@ -252,15 +253,26 @@ def main():
     time.sleep(0.25)
     launches0 = B.splotch_launch_count()
     B.splotch_profile_enable(True)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    # L2: a step streams the particle arrays and the workspace (splat records + pair list).  When that is at least twice
+    # the 126 MB L2 nothing of one step survives into the next and no flush is needed; a smaller scene (C1) gets a 256 MB
+    # fill between steps, outside the per-step event pairs, and its step time is the sum of the pairs.
+    touched = w.n * 24 + sc.workspace.numel()
+    need_flush = touched < 2 * L2_BYTES
+    flushbuf = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if need_flush else None
+    l2_note = (f"{touched / 1e6:.0f} MB touched per step < 2 x L2: 256 MB fill between steps, outside the timed event pairs" if need_flush else
+               f"inputs + workspace ({touched / 1e9:.2f} GB per step) exceed the 126 MB L2 many times over; no flush needed")
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     barrier()
-    ev[0].record()
     for k in range(args.steps):
+        if need_flush:
+            flushbuf.fill_(k & 255)
+        ev0[k].record()
         step()
-        ev[k + 1].record()                         # one event per step: median and best beside the mean
+        ev1[k].record()                            # one event pair per step: median and best beside the mean
     barrier()
-    ms_total = ev[0].elapsed_time(ev[-1])
-    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    per_step = [ev0[k].elapsed_time(ev1[k]) for k in range(args.steps)]
+    ms_total = sum(per_step) if need_flush else ev0[0].elapsed_time(ev1[-1])
     stage_ms, prof_calls = B.splotch_profile_read()
     B.splotch_profile_enable(False)
     launches = B.splotch_launch_count() - launches0
@@ -401,7 +413,7 @@ def main():
                     data="synthetic",
                     config=dict(workload=wl,
                                 parallelism=f"particle shards x{world} + all-reduce of raw S" if world > 1 else "single GPU",
-                                l2="inputs (particle arrays + splat records + pair list) exceed the 126 MB L2 many times over; no flush needed",
+                                l2=l2_note,
                                 seed=w.seed, visible=vis, pairs=pairs, pixel_updates=updates, updates_per_particle=updates / w.n,
                                 frames_per_step=n_frames, ms_per_frame=ms_frame,
                                 pixels_per_s=cam.width * cam.height / (ms_frame * 1e-3),
