@@ -59,12 +59,20 @@ constexpr int kFlagRing = 2 * kQueue / kMmaBatch;
 // ~2^-25 per MMA (measured on C3: -7e-5 with ~3700 MMAs per accumulator between flushes).  One unit of 4096 list
 // entries (~900 MMAs) keeps it near 1e-5, a tenth of the parity tolerance, for ~4 % more flush work.
 constexpr int kUnitsPerTicket = 1;
-// A batch whose 16 splats all have |a_c| <= kFaintAmp runs as ONE TF32 product per K step (operands rounded to nearest
-// TF32, no lo parts: a third of the MMAs, no operand split).  A single term is then off by at most
-// 2^-11 a_c w <= 3.8e-6 (4 % of the parity tolerance), and the roundings of different splats are independent and
-// zero-mean, so a pixel that sums N such terms is off by ~ 1.2e-4 sqrt(sum (a w)^2) <= 1.2e-4 sqrt(kFaintAmp S): 1.1e-5 at
-// S = 1 (all configs have a_c ~ 1e-5: ~4e-7).  Any brighter splat in the batch keeps the three-product split (2^-21 per term).
-constexpr float kFaintAmp = 0.0078125f;   // 2^-7
+// A batch whose 16 splats all have |a_c| <= kFaintAmp runs as ONE TF32 product per K step (operands cut to TF32, no lo
+// parts: a third of the MMAs, no operand split).  The cut is a DITHERED rounding (dither_tf32 below): a 13-bit offset that
+// depends on the splat's queue position, the work unit and the thread, never on the value, is added to the bit pattern
+// before the tensor core drops the 13 low bits.  Each operand is then unbiased (the expected value of the cut number is the
+// number itself) whatever the input is, and the errors of different splats cancel by construction: N coincident
+// splats, whose operand bits are all equal, do not repeat one rounding error N times (round-to-nearest does: up to
+// 2 x 2^-11 relative per term, the same sign every time, 5.5 x the parity tolerance at S = 1.2;
+// tests/test_gpu_parity.py::test_tensor_path_coincident_and_lattice_faint_splats).  Bounds: one term a w is off by less
+// than 2^-9 a w <= 9.6e-7 (two operands, under one TF32 ulp = 2^-10 relative each); the error of an operand has variance
+// f (1 - f) ulp^2 <= ulp^2 / 4 (f = the dropped fraction), so a pixel summing N terms is off by about
+// 2^-10.5 sqrt(sum (a w)^2) <= 6.9e-4 sqrt(kFaintAmp S) = 1.5e-5 sqrt(S) rms at the very worst (every amplitude at the
+// threshold, every fraction 1/2): 6 sigma stay inside 1e-4 max(1, S).  All configs have a_c ~ 1e-5.  Any brighter (or
+// non-finite) splat in the batch keeps the three-product split (2^-21 per term, exact enough for any sum).
+constexpr float kFaintAmp = 0.00048828125f;   // 2^-11
 constexpr int kTmemCols = 256;
 constexpr int kDCol = 0;                  // D_g at columns 64 g .. 64 g + 63
 constexpr int kACol = 128;                // A at 128 + 64 buf + 32 g + 16 (hi | lo) + k
@@ -166,9 +174,11 @@ __device__ __forceinline__ void queue_put(SmemMma &sm, uint32_t s, float sx, flo
 
 // v = hi + lo for both halves of a packed pair (Veltkamp split with 2^13 + 1: hi has 11 significant bits,
 // i.e. it is a TF32 number; lo = v - hi is exact; the tensor core ignores the 13 low bits of lo)
-// nearest TF32 (ties away) of a finite value well inside the fp32 range: add half a TF32 ulp to the bit pattern; the
-// tensor core ignores the 13 low bits.  (cvt.rna.tf32.f32 does the same plus an inf/nan test, two instructions.)
-__device__ __forceinline__ uint32_t round_tf32(float v) { return __float_as_uint(v) + 0x1000u; }
+// Dithered cut to TF32 of a finite value well inside the fp32 range: the tensor core ignores the 13 low bits of an
+// operand, so adding t >> 19 (13 bits, uniform over the splats of a Weyl sequence t) to the bit pattern rounds the value up
+// with probability (dropped fraction) and down otherwise.  t is never a function of v.
+constexpr uint32_t kDitherStride = 0x9E3779B1u;      // 2^32 / golden ratio, odd
+__device__ __forceinline__ uint32_t dither_tf32(float v, uint32_t t) { return __float_as_uint(v) + (t >> 19); }
 
 __device__ __forceinline__ void split_tf32x2(float2 v, float2 &hi, float2 &lo)
 {
@@ -221,6 +231,18 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;");
     }
+
+    // dither of the faint path: splat number p of this CTA's queue, in work unit (ticket) u, gets
+    // t = (p + u k1) * kDitherStride + dither_salt in this thread.  Over the splats t walks the golden-ratio Weyl sequence,
+    // whose discrepancy is about 2 / N: of N coincident operands the share that is rounded up differs from the dropped
+    // fraction by ~2 / N, i.e. their SUM is off by about two TF32 ulps of one operand however large N is (a random dither
+    // would give sqrt(N); a per-thread stride can be degenerate).  The per-thread salt only shifts the sequence, so that
+    // the A and B producers, the channels and the pixels do not all round up for the same splats.
+    uint32_t dither_salt = (uint32_t)tid * 0x85EBCA6Bu;
+    dither_salt ^= dither_salt >> 15;
+    dither_salt *= 0xC2B2AE35u;
+    dither_salt ^= dither_salt >> 16;
+    uint32_t dither_unit = 0u;
 
     uint32_t uses0 = 0u, uses1 = 0u;                      // batches issued into buffer 0 / 1
     uint32_t n_batches = 0;                               // batches so far (buffer = parity)
@@ -283,6 +305,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                     // channel-0 warp computes, a named barrier, the other two read) removes two thirds of the MUFU work but
                     // puts the three warps in series: measured K3t 96 -> 105 ms on C3; the batch pipeline is latency-bound.
                     const uint32_t a = lane_addr + kACol + buf * 64 + grp * 32;
+                    const uint32_t t0 = (q_head + dither_unit) * kDitherStride + dither_salt;   // splat i of the batch: t0 + i * kDitherStride
 #pragma unroll
                     for (int half = 0; half < n_splats / 8; ++half) {              // 8 splats at a time: two splats per step, f32x2 arithmetic
                         uint32_t hi[8], lo[8];
@@ -298,7 +321,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                                 hi[2 * k] = __float_as_uint(h.x);  hi[2 * k + 1] = __float_as_uint(h.y);
                                 lo[2 * k] = __float_as_uint(l.x);  lo[2 * k + 1] = __float_as_uint(l.y);
                             } else {
-                                hi[2 * k] = round_tf32(v.x);  hi[2 * k + 1] = round_tf32(v.y);
+                                hi[2 * k] = dither_tf32(v.x, t0 + (uint32_t)(8 * half + 2 * k) * kDitherStride);
+                                hi[2 * k + 1] = dither_tf32(v.y, t0 + (uint32_t)(8 * half + 2 * k + 1) * kDitherStride);
                             }
                         }
                         tmem_st8(a + 8 * half, hi);                                // faint splats 16..31 land in the columns of the lo parts
@@ -312,6 +336,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                     const float2 yy = make_float2(y, y);
                     const uint32_t qp = (q_head & (kQueue - 1)) >> 1;
                     const float4 *qg = &sm.w.qBg[qp], *qm = &sm.w.qBm[qp];
+                    const uint32_t t0 = (q_head + dither_unit) * kDitherStride + dither_salt;
 #pragma unroll
                     for (int qq = 0; qq < n_splats / 8; ++qq) {
                         const int q4 = 2 * b_half + (qq & 1) + 4 * (qq >> 1);     // group of 4 splats = 2 pairs; this warp's 8 of every 16
@@ -328,7 +353,8 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
                             const float2 f1 = make_float2(c1.x >= thr ? 1.0f : 0.0f, c1.y >= thr ? 1.0f : 0.0f);
                             float2 h, l = make_float2(0.0f, 0.0f);
                             if (bright) split_tf32x2(gy, h, l);
-                            else h = make_float2(__uint_as_float(round_tf32(gy.x)), __uint_as_float(round_tf32(gy.y)));
+                            else h = make_float2(__uint_as_float(dither_tf32(gy.x, t0 + (uint32_t)(4 * q4 + 2 * k) * kDitherStride)),
+                                                 __uint_as_float(dither_tf32(gy.y, t0 + (uint32_t)(4 * q4 + 2 * k + 1) * kDitherStride)));
                             bh[0][k] = __fmul2_rn(h, f0);  bl[0][k] = __fmul2_rn(l, f0);
                             bh[1][k] = __fmul2_rn(h, f1);  bl[1][k] = __fmul2_rn(l, f1);
                         }
@@ -452,6 +478,7 @@ raster_additive_mma_kernel(const SplatAdd *__restrict__ records, uint32_t *__res
         }
         __syncthreads();
         if (sm.ticket * (uint32_t)kUnitsPerTicket >= n_units) break;
+        dither_unit = sm.ticket * 0x632BE5ABu;
         const int n_ranges = sm.n_ranges;
         for (int r = 0; r < n_ranges; ++r) {
             const int bin = sm.range[r].bin;
