@@ -164,6 +164,18 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def spawn_command(n_gpus: int, argv, port: int = 0):
+    """The torchrun command line that `python bench.py --gpus N <argv>` re-executes itself under: the driver's own launch
+    line (one rank per GPU, rendezvous on 127.0.0.1).  port 0 = pick a free one."""
+    if not port:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -190,6 +202,20 @@ def main():
         if rank == 0:
             run_reference(args)
         return 0
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` outside torchrun: start the N ranks ourselves (one process per GPU), so that the
+        # plain command and the driver's torchrun command run the same job.  Rank 0 of the child job prints the line.
+        import subprocess
+        import torch
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: this node has {torch.cuda.device_count()} CUDA device(s)")
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")                  # the communicator log (rings / NVLS) goes to stderr
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        return subprocess.call(spawn_command(args.gpus, sys.argv[1:]), env=env)
+    if args.gpus != world:
+        log(f"[bench] --gpus {args.gpus} but WORLD_SIZE={world}: the launcher decides; running {world} rank(s)")
 
     import torch
     import torch.distributed as dist

@@ -115,3 +115,21 @@ def test_sharding_refuses_absorb_mode():
     w = workloads.make("C4", 100, width=32, height=32)
     with pytest.raises((ValueError, RuntimeError)):
         multi.ShardedScene(w, "cuda:0")
+
+
+def test_bench_spawn_command_is_the_drivers_launch_line():
+    """`python bench.py --gpus N` outside torchrun re-executes itself as one rank per GPU with the rendezvous on 127.0.0.1:
+    the command it builds is the launch line the driver uses, with the user's arguments passed through."""
+    import importlib.util
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "2", "--warmup", "3"])
+    assert cmd[:3] == [sys.executable, "-m", "torch.distributed.run"]
+    assert "--nnodes=1" in cmd and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and int(cmd[cmd.index("--master-port") + 1]) > 0
+    k = cmd.index(os.path.join(root, "bench.py"))
+    assert cmd[k + 1:] == ["--gpus", "4", "--steps", "2", "--warmup", "3"]
